@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py — decode GB/s of the ACEAPEX token stream on B200 (match phase and end-to-end) vs the HBM roofline.
+
+One "step" = one pass of the whole hot path (index, scan, literal scatter, bucketing, all match waves) over one
+compressed buffer that is already resident in HBM.  Prints ONE JSON line.
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+Workloads are BASELINE.json's synthetic configs (workloads/gen.c), encoded by the CPU oracle encoder; the
+encoded stream is cached under $ACEAPEX_CACHE (default /tmp/aceapex_cache) for the lifetime of the box.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+MiB = 1 << 20
+# name -> (generator, bytes, seed offset, encoder settings); BASELINE.json configs[0..4]
+WORKLOADS = {
+    "synth4m":   dict(kind="markov", n=4 * MiB, seed=0, enc=dict()),
+    "text256m":  dict(kind="text", n=256 * MiB, seed=1, enc=dict()),
+    "fastq1g":   dict(kind="fastq", n=1024 * MiB, seed=2, enc=dict()),
+    "text1g_d4": dict(kind="text", n=1024 * MiB, seed=1, enc=dict(depth_limit=4)),
+    "stress2g":  dict(kind="stress", n=2048 * MiB, seed=4, enc=dict()),
+}
+DEFAULT_WORKLOAD = "text256m"
+BASE_SEED = 260604268
+PAPER_CONTEXT = {"h100_match_phase_gbs": {"enwik9": 44.0, "fastq": 20.3, "enwik9_depth10": 77.2},
+                 "source": "PAPER.md:187-188, :206 (one H100 SXM; context, not the target)"}
+
+
+def load_workload(name: str, size_mb: int | None = None, enc_override: dict | None = None):
+    """Returns (raw bytes, encoded stream) for a BASELINE config; both are produced on the CPU (generator + oracle
+    encoder) and cached on local disk."""
+    import oracle
+    import workloads
+    w = WORKLOADS[name]
+    n = w["n"] if size_mb is None else size_mb * MiB
+    enc = dict(w["enc"])
+    if enc_override:
+        enc.update(enc_override)
+    cache = os.environ.get("ACEAPEX_CACHE", "/tmp/aceapex_cache")
+    tag = f"{w['kind']}_{n}_{w['seed']}_" + "_".join(f"{k}{v}" for k, v in sorted(enc.items()))
+    f_raw, f_comp = os.path.join(cache, tag + ".raw.npy"), os.path.join(cache, tag + ".comp.npy")
+    if os.path.exists(f_raw) and os.path.exists(f_comp):
+        try:
+            return np.load(f_raw), np.load(f_comp)
+        except Exception:
+            pass
+    raw = workloads.generate(w["kind"], n, BASE_SEED + w["seed"])
+    comp = oracle.encode(raw, **enc)
+    try:
+        os.makedirs(cache, exist_ok=True)
+        for f, a in ((f_raw, raw), (f_comp, comp)):
+            np.save(f + ".tmp.npy", a)
+            os.replace(f + ".tmp.npy", f)
+    except OSError:
+        pass
+    return raw, comp
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_ev = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_ev.is_set():
+            try:
+                o = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                   capture_output=True, text=True, timeout=5).stdout.strip()
+                if o:
+                    self.rows.append([x.strip() for x in o.split(",")])
+            except Exception:
+                pass
+            self._stop_ev.wait(0.1)
+
+    def finish(self) -> dict:
+        self._stop_ev.set()
+        self.join(timeout=6)
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower().startswith("active")})
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def time_oracle(comp: np.ndarray, raw_size: int, budget_s: float = 20.0) -> dict:
+    """The oracle decoder as it stands, on the host cores: sequential (the definition) and block-parallel."""
+    import oracle
+    cores = host_cores()
+    out = np.zeros(raw_size, dtype=np.uint8)                      # pre-faulted
+    best = {}
+    for label, th in (("seq", 0), ("mt", cores)):
+        t_best, spent, reps = None, 0.0, 0
+        while reps < 3 and spent < budget_s / 2:
+            t0 = time.perf_counter()
+            oracle.decode(comp, threads=th, out=out)
+            dt = time.perf_counter() - t0
+            t_best = dt if t_best is None else min(t_best, dt)
+            spent += dt
+            reps += 1
+        best[label] = raw_size / t_best / 1e9
+    return {"value": round(best["mt"], 3), "unit": "GB/s", "cores": cores, "kind": "oracle",
+            "seq_1thread_gbs": round(best["seq"], 3),
+            "sample": f"whole stream ({raw_size} B), best of <=3: oracle.decode sequential and block-parallel on {cores} threads"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    raw, comp = load_workload(args.workload, args.size_mb)
+    import oracle
+    cores = host_cores()
+    out = np.zeros(raw.size, dtype=np.uint8)
+    for _ in range(args.warmup):
+        oracle.decode(comp, threads=cores, out=out)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.decode(comp, threads=cores, out=out)
+    dt = (time.perf_counter() - t0) / args.steps
+    assert np.array_equal(out, raw)
+    v = raw.size / dt / 1e9
+    line = {"impl": "reference", "metric": "decode GB/s (decompressed bytes / s), CPU oracle block-parallel decoder",
+            "value": round(v, 3), "unit": "GB/s", "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8",
+            "data": "synthetic", "config": {"workload": args.workload, "raw_bytes": int(raw.size), "comp_bytes": int(comp.size)},
+            "cpu_baseline": {"value": round(v, 3), "unit": "GB/s", "cores": cores, "kind": "oracle",
+                             "sample": f"whole stream, oracle.decode on {cores} threads"},
+            "e2e": {"value": round(v, 3), "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def measured_peak() -> tuple[float, str]:
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_04268_b200 as ax
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))   # timing plumbing only: replicas, no data-path collective
+    dev = torch.device("cuda", local)
+
+    raw, comp = load_workload(args.workload, args.size_mb)
+    N = raw.size
+    plan = ax.Plan(comp.ctypes.data, comp.size, local)
+    if args.strategy != "auto":
+        plan.set_strategy({"launch": 1, "graph": 2, "persistent": 3}[args.strategy])
+    comp_host = torch.from_numpy(comp).pin_memory()
+    out_host = torch.empty(max(N, 1), dtype=torch.uint8).pin_memory()
+    comp_dev = comp_host.to(dev)
+    comp_dev2 = torch.empty_like(comp_dev)                        # staging target of the end-to-end (host buffer) arm
+    out_dev = torch.zeros(max(plan.out_bytes, 16), dtype=torch.uint8, device=dev)
+    scratch = torch.empty(max(plan.scratch_bytes, 16), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    sp = stream.cuda_stream
+
+    def decode(phases=ax.PHASE_ALL):
+        plan.decode(comp_dev.data_ptr(), out_dev.data_ptr(), out_dev.numel(), scratch.data_ptr(), scratch.numel(), phases, sp)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed(fn, steps, pre=None):
+        """Device time of `steps` calls of fn (CUDA events on the launching stream); `pre` runs untimed before each."""
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        barrier()
+        for s, e in evs:
+            if pre:
+                pre()
+            s.record(stream)
+            fn()
+            e.record(stream)
+        barrier()
+        ms = [s.elapsed_time(e) for s, e in evs]
+        return sum(ms), ms
+
+    # ---- correctness first: GPU bytes == generator bytes (pinned to the oracle by the round-trip tests)
+    decode()
+    st = plan.stats(scratch.data_ptr())
+    got = out_dev[:N].cpu().numpy()
+    if not np.array_equal(got, raw):
+        raise SystemExit("bench.py: GPU decode is not bit-exact")
+    launches_per_step = st["n_launches"]
+    for _ in range(max(args.warmup, 3) - 1):
+        decode()
+    sampler = ClockSampler(local)
+    sampler.start()
+    tot_ms, all_ms = timed(decode, args.steps, pre=lambda: out_dev.zero_())                      # whole hot path
+    decode(ax.PHASE_PRE)
+    mt_ms, match_ms = timed(lambda: decode(ax.PHASE_MATCH), args.steps)                           # match waves alone
+    pt_ms, pre_ms = timed(lambda: decode(ax.PHASE_PRE), args.steps)                               # index+scan+literals+bucketing
+    clocks = sampler.finish()
+    # ---- end to end through the C ABI with HOST buffers (H2D + decode + D2H inside the timed region)
+    def e2e():
+        plan.decode_host(comp_host.data_ptr(), comp.size, out_host.data_ptr(), out_host.numel(), comp_dev2.data_ptr(),
+                         out_dev.data_ptr(), out_dev.numel(), scratch.data_ptr(), scratch.numel(), sp)
+    e2e()
+    torch.cuda.synchronize(dev)
+    if not np.array_equal(out_host.numpy()[:N], raw):
+        raise SystemExit("bench.py: host-buffer decode is not bit-exact")
+    e2e_steps = max(1, min(args.steps, 5))
+    e2e_tot, _ = timed(e2e, e2e_steps)
+
+    def maxr(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+    tot_ms, mt_ms, pt_ms, e2e_tot = maxr(tot_ms), maxr(mt_ms), maxr(pt_ms), maxr(e2e_tot)
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        ms_step, ms_match, ms_pre, ms_e2e = tot_ms / args.steps, mt_ms / args.steps, pt_ms / args.steps, e2e_tot / e2e_steps
+        C, M, Msrc, nm = st["comp_bytes"], st["match_bytes"], st["match_src_bytes"], st["n_match"]
+        b_e2e = C + Msrc + N                                     # north_star: compressed read + match source read + output written
+        b_match = 6 * nm + Msrc + M                              # off+len entries, source bytes, match bytes written
+        gbs = lambda b, ms: b / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        cnt, byt = plan.depth_hist()
+        waves = [c for c in cnt[1:]]
+        line = {
+            "metric": "decode GB/s on 1 B200 (decompressed bytes / s, whole hot path, compressed stream resident in HBM)",
+            "value": round(world * gbs(N, ms_step), 2), "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+            "config": {"workload": args.workload, "raw_bytes": int(N), "comp_bytes": int(C), "n_seq": st["n_seq"], "n_match": nm,
+                       "lit_bytes": st["lit_bytes"], "match_src_bytes": Msrc, "block_size": st["block_size"],
+                       "max_depth": st["max_depth"], "depth_limit": st["depth_limit"], "flattened": bool(st["flags"] & 1),
+                       "wave_strategy": ax.STRATEGY_NAMES[st["strategy"]], "replicas": world,
+                       "l2": "inputs larger than L2 (no flush)" if C + N > 256 * MiB else "small config: L2-resident, correctness only",
+                       "output_rezeroed_between_steps": True},
+            "match_phase": {"gbs": round(gbs(N, ms_match), 2), "ms": round(ms_match, 4), "algorithmic_bytes": int(b_match),
+                            "achieved_gbs": round(gbs(b_match, ms_match), 1), "frac_of_measured_peak": round(gbs(b_match, ms_match) / peak, 4),
+                            "frac_of_nominal_8000": round(gbs(b_match, ms_match) / 8000.0, 4)},
+            "end_to_end_device": {"gbs": round(gbs(N, ms_step), 2), "ms": round(ms_step, 4), "algorithmic_bytes": int(b_e2e),
+                                  "achieved_gbs": round(gbs(b_e2e, ms_step), 1), "frac_of_measured_peak": round(gbs(b_e2e, ms_step) / peak, 4),
+                                  "frac_of_nominal_8000": round(gbs(b_e2e, ms_step) / 8000.0, 4)},
+            "pre_phase": {"ms": round(ms_pre, 4)},
+            "waves": {"n_waves": len(waves), "matches_per_wave_min_med_max": [int(min(waves)), int(sorted(waves)[len(waves) // 2]), int(max(waves))] if waves else [],
+                      "depth_hist_head": [[d, int(cnt[d]), int(byt[d])] for d in range(min(len(cnt), 9))]},
+            "roofline": {"bound": "hbm", "kernel": "match waves (k_wave / k_waves_persistent, all depths of one step)",
+                         "achieved": round(gbs(b_match, ms_match), 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                         "frac": round(gbs(b_match, ms_match) / peak, 4), "traffic": None},
+            "e2e": {"value": round(world * gbs(N, ms_e2e), 2), "unit": "GB/s", "h2d_bytes_per_step": int(C), "d2h_bytes_per_step": int(N),
+                    "ms": round(ms_e2e, 3), "steps": e2e_steps},
+            "gpu_launches": int(launches_per_step * args.steps),
+            "clocks": clocks, "paper_context": PAPER_CONTEXT,
+        }
+        if world == 1 and not args.no_cpu:
+            line["cpu_baseline"] = time_oracle(comp, N)
+        print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--size-mb", type=int, default=None, help="development override of the workload size")
+    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,310 @@
+// api.cu — the C ABI of libaceapex (include/aceapex.h): plan (host-side header/directory validation, scratch
+// layout, wave strategy), decode (kernel sequencing on the caller's stream), stats.
+#include "../../include/aceapex.h"
+#include "common.cuh"
+
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace ax {
+void launch_index(const Params& P, int n_sm, cudaStream_t st);
+void launch_pre(const Params& P, int grid, cudaStream_t st);
+cudaError_t pre_configure();
+size_t pre_smem_bytes();
+int pre_max_ctas_per_sm();
+int match_max_ctas_per_sm();
+cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
+cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
+}  // namespace ax
+
+using namespace ax;
+
+struct GraphSlot {
+    const void* comp; void* out; void* scratch; unsigned phases; int strategy;
+    cudaGraphExec_t exec; uint32_t n_launches;
+};
+
+struct aceapex_plan_s {
+    // header (docs/FORMAT.md)
+    uint32_t flags, block_size, n_blocks, min_match, depth_limit, max_depth;
+    uint64_t raw_size, total_seq, total_lit, comp_bytes, n_match;
+    std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
+    uint32_t n_tiles;
+    // device facts
+    int device, n_sm, pre_grid, match_ctas_per_sm;
+    // scratch layout (byte offsets)
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_dst, o_off, o_len, scratch_bytes;
+    int strategy_auto, strategy_forced;
+    uint32_t last_launches; int last_strategy;
+    int last_cuda;
+    cudaStream_t last_stream;
+    std::vector<GraphSlot> graphs;
+};
+
+static inline uint32_t rd32(const uint8_t* p) { uint32_t v; memcpy(&v, p, 4); return v; }
+static inline uint64_t rd64(const uint8_t* p) { uint64_t v; memcpy(&v, p, 8); return v; }
+static inline size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+extern "C" const char* aceapex_strerror(int code) {
+    switch (code) {
+        case ACEAPEX_OK: return "ok";
+        case ACEAPEX_E_MAGIC: return "bad magic";
+        case ACEAPEX_E_VERSION: return "unsupported version";
+        case ACEAPEX_E_TRUNCATED: return "compressed buffer truncated";
+        case ACEAPEX_E_HEADER: return "inconsistent header or directory";
+        case ACEAPEX_E_CAPACITY: return "output or scratch capacity too small";
+        case ACEAPEX_E_ALIGN: return "device pointer not 16-byte aligned";
+        case ACEAPEX_E_CUDA: return "CUDA runtime error";
+        case ACEAPEX_E_ARG: return "bad argument";
+        case ACEAPEX_E_STREAM: return "token stream fault detected on the device";
+        case ACEAPEX_E_NOMEM: return "host allocation failed";
+        default: return "unknown error";
+    }
+}
+
+// Wave strategy from the per-depth counts: few waves -> one launch each;
+// many waves -> persistent kernel with grid barriers (a launch costs more than a barrier).
+static int choose_strategy(const aceapex_plan_t* p) {
+    const char* e = getenv("ACEAPEX_WAVES");
+    if (e) {
+        if (!strcmp(e, "launch")) return ACEAPEX_WAVES_LAUNCH;
+        if (!strcmp(e, "graph")) return ACEAPEX_WAVES_GRAPH;
+        if (!strcmp(e, "persistent")) return ACEAPEX_WAVES_PERSISTENT;
+    }
+    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
+}
+
+extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
+    if (!out) return ACEAPEX_E_ARG;
+    *out = nullptr;
+    if (!comp_host || device < 0) return ACEAPEX_E_ARG;
+    const uint8_t* c = static_cast<const uint8_t*>(comp_host);
+    if (comp_bytes < HDR_BYTES) return ACEAPEX_E_TRUNCATED;
+    if (memcmp(c, "ACEAPEX1", 8) != 0) return ACEAPEX_E_MAGIC;
+    if (rd32(c + 8) != 1) return ACEAPEX_E_VERSION;
+    aceapex_plan_t* p = new (std::nothrow) aceapex_plan_t();
+    if (!p) return ACEAPEX_E_NOMEM;
+    int rc = ACEAPEX_OK;
+    do {
+        p->flags = rd32(c + 12); p->raw_size = rd64(c + 16); p->block_size = rd32(c + 24); p->n_blocks = rd32(c + 28);
+        p->min_match = rd32(c + 32); p->depth_limit = rd32(c + 36); p->max_depth = rd32(c + 40);
+        p->total_seq = rd64(c + 48); p->total_lit = rd64(c + 56); p->comp_bytes = comp_bytes;
+        if (p->block_size == 0 || p->block_size > (1u << 28) || p->raw_size > 0xFFFFFFFFull || p->max_depth > 65535 ||
+            p->min_match == 0 || p->total_seq >= 0xFFFFFFF0ull || !(p->flags & FLAG_HAS_DEP)) { rc = ACEAPEX_E_HEADER; break; }
+        const uint64_t nb = (p->raw_size + p->block_size - 1) / p->block_size;
+        if (nb != p->n_blocks) { rc = ACEAPEX_E_HEADER; break; }
+        const uint64_t meta = HDR_BYTES + (uint64_t)DIR_BYTES * nb + (uint64_t)HIST_BYTES * (p->max_depth + 1ull);
+        const uint64_t meta_p = (meta + 127) & ~127ull;
+        if (meta_p > comp_bytes) { rc = ACEAPEX_E_TRUNCATED; break; }
+        const uint8_t* dir = c + HDR_BYTES;
+        const uint8_t* hist = dir + DIR_BYTES * nb;
+        uint64_t prev_end = meta_p, ts = 0, tl = 0, tiles = 0;
+        for (uint64_t b = 0; b < nb && rc == ACEAPEX_OK; ++b) {
+            const uint64_t po = rd64(dir + 16 * b); const uint32_t ns = rd32(dir + 16 * b + 8), nl = rd32(dir + 16 * b + 12);
+            if ((po & 127) || po < prev_end || ns == 0) { rc = ACEAPEX_E_HEADER; break; }
+            const uint64_t bytes = 3 * pad16(2ull * ns) + pad16(4ull * ns) + pad16(nl);
+            if (po > comp_bytes || bytes > comp_bytes - po) { rc = ACEAPEX_E_TRUNCATED; break; }
+            prev_end = po + bytes; ts += ns; tl += nl; tiles += (ns + TILE - 1) / TILE;
+        }
+        if (rc) break;
+        if (ts != p->total_seq || tl != p->total_lit || tl > p->raw_size || tiles > 0xFFFFFFF0ull) { rc = ACEAPEX_E_HEADER; break; }
+        p->n_tiles = (uint32_t)tiles;
+        p->hist_cnt.resize(p->max_depth + 1); p->hist_bytes.resize(p->max_depth + 1);
+        uint64_t nm = 0, mb = 0;
+        for (uint32_t d = 0; d <= p->max_depth; ++d) {
+            p->hist_cnt[d] = rd32(hist + 16 * d); p->hist_bytes[d] = rd64(hist + 16 * d + 8);
+            if (d) { nm += p->hist_cnt[d]; mb += p->hist_bytes[d]; }
+        }
+        if (nm > p->total_seq || p->hist_bytes[0] != p->total_lit || mb + p->total_lit != p->raw_size ||
+            (p->max_depth && p->hist_cnt[p->max_depth] == 0)) { rc = ACEAPEX_E_HEADER; break; }
+        p->n_match = nm;
+        // device facts
+        cudaDeviceProp prop;
+        int cur = -1;
+        cudaError_t ce = cudaGetDevice(&cur);
+        if (ce == cudaSuccess) ce = cudaSetDevice(device);
+        if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, device);
+        if (ce == cudaSuccess) ce = pre_configure();
+        if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
+        p->device = device; p->n_sm = prop.multiProcessorCount;
+        int pre_occ = pre_max_ctas_per_sm(); if (pre_occ < 1) pre_occ = 1;
+        p->pre_grid = p->n_sm * pre_occ;
+        p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
+        if (cur >= 0 && cur != device) cudaSetDevice(cur);
+        // scratch layout
+        size_t o = 0;
+        p->o_status = o; o += up256(sizeof(Status));
+        p->o_wave_off = o; o += up256(4ull * (p->max_depth + 2));
+        p->o_cursor = o; o += up256(4ull * (p->max_depth + 2));
+        p->o_blocks = o; o += up256(sizeof(BlockDesc) * (size_t)nb);
+        p->o_tiles = o; o += up256(8ull * p->n_tiles);
+        p->o_dst = o; o += up256(4ull * nm);
+        p->o_off = o; o += up256(4ull * nm);
+        p->o_len = o; o += up256(2ull * nm);
+        p->scratch_bytes = o;
+        p->strategy_forced = ACEAPEX_WAVES_AUTO;
+        p->strategy_auto = choose_strategy(p);
+        p->last_strategy = p->strategy_auto;
+    } while (0);
+    if (rc) { delete p; return rc; }
+    *out = p;
+    return ACEAPEX_OK;
+}
+
+extern "C" size_t aceapex_raw_bytes(const aceapex_plan_t* p) { return p ? (size_t)p->raw_size : 0; }
+extern "C" size_t aceapex_out_bytes(const aceapex_plan_t* p) { return p ? (size_t)((p->raw_size + 15) & ~15ull) : 0; }
+extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p->scratch_bytes : 0; }
+extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
+
+extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PERSISTENT) return ACEAPEX_E_ARG;
+    p->strategy_forced = s;
+    return ACEAPEX_OK;
+}
+
+static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* out_dev, void* scratch_dev) {
+    Params P;
+    uint8_t* s = static_cast<uint8_t*>(scratch_dev);
+    P.comp = static_cast<const uint8_t*>(comp_dev); P.out = static_cast<uint8_t*>(out_dev);
+    P.status = reinterpret_cast<Status*>(s + p->o_status);
+    P.wave_off = reinterpret_cast<uint32_t*>(s + p->o_wave_off);
+    P.cursor = reinterpret_cast<uint32_t*>(s + p->o_cursor);
+    P.blocks = reinterpret_cast<BlockDesc*>(s + p->o_blocks);
+    P.tile_state = reinterpret_cast<unsigned long long*>(s + p->o_tiles);
+    P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
+    P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
+    P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
+    P.raw_size = p->raw_size; P.block_size = p->block_size; P.n_blocks = p->n_blocks; P.n_tiles = p->n_tiles;
+    P.max_depth = p->max_depth; P.min_match = p->min_match; P.n_match = (uint32_t)p->n_match;
+    return P;
+}
+
+// Enqueue the kernels of one decode on `st`; returns the number of kernel launches through *n_launch.
+static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, int strategy, cudaStream_t st, uint32_t* n_launch) {
+    uint32_t n = 0;
+    if (p->n_blocks == 0) { *n_launch = 0; return cudaSuccess; }
+    if (phases & ACEAPEX_PHASE_PRE) {
+        launch_index(P, p->n_sm, st); ++n;
+        launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
+        if (strategy == ACEAPEX_WAVES_PERSISTENT) {
+            cudaError_t e = launch_waves_persistent(P, 1, p->max_depth, p->n_sm * p->match_ctas_per_sm, st);
+            if (e != cudaSuccess) return e;
+            ++n;
+        } else {
+            for (uint32_t d = 1; d <= p->max_depth; ++d) {
+                cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], p->n_sm * p->match_ctas_per_sm * 4, st);
+                if (e != cudaSuccess) return e;
+                if (p->hist_cnt[d]) ++n;
+            }
+        }
+    }
+    *n_launch = n;
+    return cudaGetLastError();
+}
+
+extern "C" int aceapex_decode(aceapex_plan_t* p, const void* comp_dev, void* out_dev, size_t out_capacity,
+                              void* scratch_dev, size_t scratch_bytes, unsigned phases, void* stream) {
+    if (!p || !(phases & ACEAPEX_PHASE_ALL) || (phases & ~(unsigned)ACEAPEX_PHASE_ALL)) return ACEAPEX_E_ARG;
+    if (p->n_blocks == 0) { p->last_launches = 0; p->last_stream = (cudaStream_t)stream; return ACEAPEX_OK; }
+    if (!comp_dev || !out_dev || !scratch_dev) return ACEAPEX_E_ARG;
+    if (out_capacity < aceapex_out_bytes(p) || scratch_bytes < p->scratch_bytes) return ACEAPEX_E_CAPACITY;
+    if (((uintptr_t)comp_dev | (uintptr_t)out_dev | (uintptr_t)scratch_dev) & 15) return ACEAPEX_E_ALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    p->last_stream = st;
+    const int strategy = p->strategy_forced != ACEAPEX_WAVES_AUTO ? p->strategy_forced : p->strategy_auto;
+    p->last_strategy = strategy;
+    const Params P = make_params(p, comp_dev, out_dev, scratch_dev);
+    cudaError_t e;
+    if (strategy != ACEAPEX_WAVES_GRAPH) {
+        e = enqueue(p, P, phases, strategy, st, &p->last_launches);
+        if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+        return ACEAPEX_OK;
+    }
+    // ---- CUDA graph: the launch sequence depends only on the plan and the three pointers; cache it
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone) {   // caller is capturing already
+        e = enqueue(p, P, phases, ACEAPEX_WAVES_LAUNCH, st, &p->last_launches);
+        if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+        return ACEAPEX_OK;
+    }
+    for (GraphSlot& g : p->graphs)
+        if (g.comp == comp_dev && g.out == out_dev && g.scratch == scratch_dev && g.phases == phases) {
+            e = cudaGraphLaunch(g.exec, st);
+            if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+            p->last_launches = g.n_launches;
+            return ACEAPEX_OK;
+        }
+    cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr; uint32_t nl = 0;
+    e = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        cudaError_t e2 = enqueue(p, P, phases, ACEAPEX_WAVES_LAUNCH, st, &nl);
+        e = cudaStreamEndCapture(st, &graph);
+        if (e2 != cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e == cudaSuccess) e = cudaGraphLaunch(exec, st);
+    if (e != cudaSuccess) { if (exec) cudaGraphExecDestroy(exec); p->last_cuda = (int)e; cudaGetLastError(); return ACEAPEX_E_CUDA; }
+    if (p->graphs.size() >= 8) { cudaGraphExecDestroy(p->graphs.front().exec); p->graphs.erase(p->graphs.begin()); }
+    p->graphs.push_back(GraphSlot{comp_dev, out_dev, scratch_dev, phases, strategy, exec, nl});
+    p->last_launches = nl;
+    return ACEAPEX_OK;
+}
+
+extern "C" int aceapex_decode_host(aceapex_plan_t* p, const void* comp_host, size_t comp_bytes, void* out_host,
+                                   size_t out_host_capacity, void* comp_dev, void* out_dev, size_t out_capacity,
+                                   void* scratch_dev, size_t scratch_bytes, void* stream) {
+    if (!p || !comp_host || (!out_host && p->raw_size)) return ACEAPEX_E_ARG;
+    if (comp_bytes != p->comp_bytes) return ACEAPEX_E_ARG;
+    if (out_host_capacity < p->raw_size) return ACEAPEX_E_CAPACITY;
+    if (p->n_blocks == 0) return ACEAPEX_OK;
+    if (!comp_dev) return ACEAPEX_E_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(comp_dev, comp_host, comp_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+    int rc = aceapex_decode(p, comp_dev, out_dev, out_capacity, scratch_dev, scratch_bytes, ACEAPEX_PHASE_ALL, stream);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(out_host, out_dev, p->raw_size, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+    return ACEAPEX_OK;
+}
+
+extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, aceapex_stats* s) {
+    if (!p || !s) return ACEAPEX_E_ARG;
+    memset(s, 0, sizeof *s);
+    s->raw_bytes = p->raw_size; s->comp_bytes = p->comp_bytes; s->lit_bytes = p->total_lit;
+    s->match_bytes = p->raw_size - p->total_lit; s->n_seq = p->total_seq; s->n_match = p->n_match;
+    s->n_blocks = p->n_blocks; s->block_size = p->block_size; s->min_match = p->min_match; s->max_depth = p->max_depth;
+    s->depth_limit = p->depth_limit; s->flags = p->flags; s->strategy = (uint32_t)p->last_strategy;
+    s->n_launches = p->last_launches;
+    if (scratch_dev && p->n_blocks) {
+        Status h;
+        cudaError_t e = cudaStreamSynchronize(p->last_stream);
+        if (e == cudaSuccess) e = cudaMemcpy(&h, static_cast<const uint8_t*>(scratch_dev) + p->o_status, sizeof h, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+        s->match_src_bytes = h.match_src_bytes; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
+        if (h.fault_flags) return ACEAPEX_E_STREAM;
+    }
+    return ACEAPEX_OK;
+}
+
+extern "C" int64_t aceapex_depth_hist(const aceapex_plan_t* p, uint64_t* n_match, uint64_t* n_bytes, uint32_t cap) {
+    if (!p) return ACEAPEX_E_ARG;
+    for (uint32_t d = 0; d <= p->max_depth && d < cap; ++d) {
+        if (n_match) n_match[d] = p->hist_cnt[d];
+        if (n_bytes) n_bytes[d] = p->hist_bytes[d];
+    }
+    return (int64_t)p->max_depth + 1;
+}
+
+extern "C" void aceapex_free(aceapex_plan_t* p) {
+    if (!p) return;
+    for (GraphSlot& g : p->graphs) cudaGraphExecDestroy(g.exec);
+    delete p;
+}

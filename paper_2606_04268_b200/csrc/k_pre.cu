@@ -1,0 +1,219 @@
+// k_pre.cu — steps a2-a5 fused: token parse, segmented exclusive length scan, literal scatter, depth bucketing.
+//   a2  per sequence: lit_len = cmd[j], mlen = len[j]                                   (§3.2)
+//   a3  dst[j] = out_base[b] + sum_{i<j}(cmd[i]+len[i]);  lsrc[j] = sum_{i<j} cmd[i]      (the sequential walk of
+//       PAPER.md:53 restated as a scan; one independent scan per 1 MB block)
+//   a4  out[dst[j] .. +cmd[j]) = lit_b[lsrc[j] ..)
+//   a5  matches grouped by dep[j] into per-depth wave lists (mdst, off, len)             (§7.1)
+// One tile = 2048 consecutive sequences of one block.  CTAs take tiles in order from a ticket counter, so a
+// tile's predecessors have always started: the per-block prefix is carried by decoupled look-back.  dst[] and
+// lsrc[] are never written to memory.
+#include "common.cuh"
+
+namespace ax {
+
+constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_MASK = 3ull << 62;
+constexpr uint32_t SAT = 0x3FFFFFFFu;   // sums saturate here (valid streams stay <= block_size <= 2^28)
+
+__device__ __forceinline__ unsigned long long pack_state(unsigned long long flag, uint32_t so, uint32_t sl) {
+    so = so > SAT ? SAT : so; sl = sl > SAT ? SAT : sl;
+    return flag | ((unsigned long long)so << 31) | (unsigned long long)sl;
+}
+__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+struct PreSmem {
+    unsigned long long warp_sum[PRE_THREADS / 32];
+    unsigned long long tile_prefix;      // (out << 32) | lit of everything before this tile in its block
+    uint32_t tile;
+    uint32_t cnt[SMEM_DEPTHS];           // per-depth count inside the tile
+    uint32_t gbase[SMEM_DEPTHS];         // per-depth start in the wave list reserved for this tile
+};
+
+__global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PreSmem& S = *reinterpret_cast<PreSmem*>(smem_raw);
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool smem_bins = (P.max_depth + 1) <= SMEM_DEPTHS;
+    if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) S.cnt[i] = 0;
+    unsigned long long src_bytes = 0;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) S.tile = atomicAdd(&P.status->ticket, 1u);
+        __syncthreads();
+        const uint32_t tile = S.tile;
+        if (tile >= P.n_tiles) break;
+        // ---- which block: last b with tile_base[b] <= tile (blocks with n_seq = 0 own no tile)
+        uint32_t lo = 0, hi = P.n_blocks - 1;
+        while (lo < hi) {
+            const uint32_t mid = (lo + hi + 1) >> 1;
+            if (P.blocks[mid].tile_base <= tile) lo = mid; else hi = mid - 1;
+        }
+        const uint32_t b = lo;
+        const BlockDesc B = P.blocks[b];
+        const uint32_t t_in_blk = tile - B.tile_base;
+        const uint32_t j0 = t_in_blk * TILE + tid * PRE_ITEMS;          // first sequence of this thread
+        // ---- a2: parse (16-byte loads; streams are padded to 16 bytes, entries past n_seq are masked)
+        uint32_t c[PRE_ITEMS], l[PRE_ITEMS], dp[PRE_ITEMS], of[PRE_ITEMS];
+        if (j0 < B.n_seq) {
+            const uint4 vc = *reinterpret_cast<const uint4*>(P.comp + B.cmd_off + 2ull * j0);
+            const uint4 vl = *reinterpret_cast<const uint4*>(P.comp + B.len_off + 2ull * j0);
+            const uint4 vd = *reinterpret_cast<const uint4*>(P.comp + B.dep_off + 2ull * j0);
+            const uint4 o0 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0);
+            const uint4 o1 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0 + 16);
+            const uint32_t wc[4] = {vc.x, vc.y, vc.z, vc.w}, wl[4] = {vl.x, vl.y, vl.z, vl.w}, wd[4] = {vd.x, vd.y, vd.z, vd.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                c[2 * k] = wc[k] & 0xFFFFu; c[2 * k + 1] = wc[k] >> 16;
+                l[2 * k] = wl[k] & 0xFFFFu; l[2 * k + 1] = wl[k] >> 16;
+                dp[2 * k] = wd[k] & 0xFFFFu; dp[2 * k + 1] = wd[k] >> 16;
+            }
+            of[0] = o0.x; of[1] = o0.y; of[2] = o0.z; of[3] = o0.w; of[4] = o1.x; of[5] = o1.y; of[6] = o1.z; of[7] = o1.w;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) if (j0 + k >= B.n_seq) { c[k] = 0; l[k] = 0; dp[k] = 0; of[k] = 0; }
+        } else {
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) { c[k] = 0; l[k] = 0; dp[k] = 0; of[k] = 0; }
+        }
+        // ---- a3: scan of (cmd+len, cmd) packed as (hi, lo) of one u64
+        unsigned long long tsum = 0;
+#pragma unroll
+        for (int k = 0; k < PRE_ITEMS; ++k) tsum += ((unsigned long long)(c[k] + l[k]) << 32) | c[k];
+        unsigned long long inc = tsum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+            if (lane >= d) inc += t;
+        }
+        if (lane == 31) S.warp_sum[warp] = inc;
+        __syncthreads();
+        unsigned long long wpre = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < PRE_THREADS / 32; ++w) {
+            const unsigned long long x = S.warp_sum[w];
+            if (w < (int)warp) wpre += x;
+            total += x;
+        }
+        if (tid == 0) {   // decoupled look-back along this block's tiles
+            const uint32_t tot_o = (uint32_t)(total >> 32), tot_l = (uint32_t)total;
+            uint32_t pre_o = 0, pre_l = 0;
+            if (t_in_blk != 0) {
+                st_relaxed(&P.tile_state[tile], pack_state(ST_AGG, tot_o, tot_l));
+                uint32_t q = tile;
+                for (;;) {
+                    --q;
+                    unsigned long long s;
+                    do { s = ld_relaxed(&P.tile_state[q]); } while ((s & ST_MASK) == 0);
+                    pre_o += (uint32_t)((s >> 31) & 0x7FFFFFFFu); pre_l += (uint32_t)(s & 0x7FFFFFFFu);
+                    if (pre_o > SAT) pre_o = SAT;
+                    if (pre_l > SAT) pre_l = SAT;
+                    if ((s & ST_MASK) == ST_INC) break;
+                }
+            }
+            st_relaxed(&P.tile_state[tile], pack_state(ST_INC, pre_o + tot_o, pre_l + tot_l));
+            S.tile_prefix = ((unsigned long long)pre_o << 32) | pre_l;
+            const bool last_tile = (t_in_blk + 1) * (uint32_t)TILE >= B.n_seq;
+            if (last_tile && (pre_o + tot_o != B.raw_len || pre_l + tot_l != B.n_lit)) raise_fault(P.status, F_BLOCK_SUM, b);
+        }
+        __syncthreads();
+        const unsigned long long ex = S.tile_prefix + wpre + (inc - tsum);
+        uint32_t pos = (uint32_t)(ex >> 32);                 // output offset inside the block
+        uint32_t lsrc = (uint32_t)ex;                        // offset inside the block's lit[]
+        const uint8_t* lit = P.comp + B.lit_off;
+        uint8_t* outb = P.out + B.out_base;
+        // ---- a4 literal scatter + a5 ranking, sequence by sequence (loop trip count is warp-uniform)
+        uint32_t rank[PRE_ITEMS];
+        uint32_t first_mask = 0;                             // bit k: this thread opened depth bin dp[k] in this tile
+#pragma unroll
+        for (int k = 0; k < PRE_ITEMS; ++k) {
+            bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len && (uint64_t)lsrc + c[k] <= B.n_lit;
+            if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
+            const uint32_t cc = ok ? c[k] : 0;
+            // literal run: short ones by their own thread, long ones by the whole warp
+            if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }
+            uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
+            while (longm) {
+                const int src_lane = __ffs(longm) - 1; longm &= longm - 1;
+                const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, src_lane), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, src_lane),
+                               n2 = __shfl_sync(0xFFFFFFFFu, cc, src_lane);
+                warp_copy(outb + p2, lit + s2, n2, lane);
+            }
+            pos += c[k]; lsrc += c[k];
+            // match: validate (I2), rank inside its depth bin
+            bool m = ok && l[k] != 0;
+            if (l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
+            if (m) {
+                const uint64_t mdst = B.out_base + pos;
+                if (of[k] >= mdst || l[k] < P.min_match) { raise_fault(P.status, F_SOURCE, b); m = false; }
+                else if (dp[k] == 0 || dp[k] > P.max_depth) { raise_fault(P.status, F_DEPTH, b); m = false; }
+            }
+            if (m) { const uint32_t dist = (uint32_t)(B.out_base + pos - of[k]); src_bytes += l[k] < dist ? l[k] : dist; }
+            const uint32_t key = m ? dp[k] : 0u;
+            const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+            const int leader = __ffs(peers) - 1;
+            uint32_t base = 0;
+            if (m && (int)lane == leader) {
+                if (smem_bins) { base = atomicAdd(&S.cnt[key], (uint32_t)__popc(peers)); if (base == 0) first_mask |= 1u << k; }
+                else base = atomicAdd(&P.cursor[key], (uint32_t)__popc(peers));
+            }
+            base = __shfl_sync(0xFFFFFFFFu, base, leader);
+            rank[k] = base + __popc(peers & ((1u << lane) - 1u));
+            of[k] = m ? of[k] : 0xFFFFFFFFu;                 // 0xFFFFFFFF marks "no entry" (a valid off is < mdst <= 2^32-1)
+            c[k] = (uint32_t)(B.out_base + pos);             // reuse c[] as mdst
+            pos += l[k];
+        }
+        if (smem_bins) {
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k)
+                if (first_mask & (1u << k)) {            // reserve this tile's slice of the depth's wave list
+                    S.gbase[dp[k]] = atomicAdd(&P.cursor[dp[k]], S.cnt[dp[k]]);
+                    S.cnt[dp[k]] = 0;                    // bin is clean again for the next tile
+                }
+            __syncthreads();
+        }
+        // ---- a5: write the wave list entries
+#pragma unroll
+        for (int k = 0; k < PRE_ITEMS; ++k) {
+            if (of[k] == 0xFFFFFFFFu) continue;
+            const uint32_t at = (smem_bins ? S.gbase[dp[k]] : 0u) + rank[k];
+            if (at >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); continue; }   // more matches than the histogram says
+            P.wl_dst[at] = c[k]; P.wl_off[at] = of[k]; P.wl_len[at] = (uint16_t)l[k];
+        }
+    }
+    // ---- M_src for the roofline report (aceapex_stats.match_src_bytes)
+#pragma unroll
+    for (int d = 16; d; d >>= 1) src_bytes += __shfl_xor_sync(0xFFFFFFFFu, src_bytes, d);
+    if (lane == 0 && src_bytes) atomicAdd(&P.status->match_src_bytes, src_bytes);
+}
+
+// After PRE: every cursor must have reached the end of its list, else the histogram lied (fault F_DEPTH).
+__global__ void k_check_cursors(Params P) {
+    const uint32_t d = blockIdx.x * blockDim.x + threadIdx.x + 1;
+    if (d <= P.max_depth && P.cursor[d] != P.wave_off[d + 1]) raise_fault(P.status, F_DEPTH, 0xFFFFFFFEu);
+}
+
+size_t pre_smem_bytes() { return sizeof(PreSmem); }
+
+cudaError_t pre_configure() {
+    return cudaFuncSetAttribute(k_pre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PreSmem));
+}
+
+int pre_max_ctas_per_sm() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pre, PRE_THREADS, sizeof(PreSmem)) != cudaSuccess) return 0;
+    return n;
+}
+
+void launch_pre(const Params& P, int grid, cudaStream_t st) {
+    if (P.n_tiles) k_pre<<<grid, PRE_THREADS, sizeof(PreSmem), st>>>(P);
+    if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
+}
+
+}  // namespace ax

@@ -1,0 +1,266 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit-exact, on the same seeded inputs.
+Every test here needs a B200 (``-m gpu``)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+import paper_2606_04268_b200 as ax
+from streams import build_stream, py_decode, py_depths, random_blocks
+
+pytestmark = pytest.mark.gpu
+
+STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]
+
+
+def gpu_decode(comp, strategy=0, check=True):
+    from paper_2606_04268_b200.torch_io import Decoder
+    d = Decoder(comp, 0, strategy)
+    try:
+        d.run()
+        out = d.output()
+        st = d.stats(check=check)
+        return out, st
+    finally:
+        d.close()
+
+
+def assert_parity(comp, raw=None, strategies=STRATS):
+    want = oracle.decode(comp)
+    rep = oracle.validate(comp)
+    for s in strategies:
+        got, st = gpu_decode(comp, s)
+        assert got.size == want.size
+        if not np.array_equal(got, want):
+            bad = np.flatnonzero(got != want)
+            raise AssertionError(f"strategy {s}: {bad.size} bytes differ, first at {bad[0]}")
+        assert st["match_src_bytes"] == rep["match_src_bytes"] and st["n_match"] == rep["n_match"]
+    if raw is not None:
+        assert np.array_equal(want, raw)
+
+
+# ---------------------------------------------------------------- hand-built streams (tests/streams.py)
+def test_paper_examples():
+    E1 = [[(b"abcdefgh", 8, 0), (b"WX", 8, 0), (b"z", 5, 26)]]
+    assert_parity(build_stream(E1, 32, flags=5))
+    E1b = [[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]]                 # flatten off: depth 2
+    assert_parity(build_stream(E1b, 32))
+    E2 = [[(b"abcdefgh", 8, 0)], [(b"", 16, 8)]]                                # PAPER.md:63 cross-block, overlap period 8
+    assert_parity(build_stream(E2, 16))
+    rng = np.random.default_rng(1)
+    lit0 = rng.integers(0, 256, 5100, dtype=np.uint8).tobytes()
+    lit1 = rng.integers(0, 256, 150, dtype=np.uint8).tobytes()
+    T1 = [[(lit0, 50, 5000), (lit1, 50, 5000), (b"tail", 0, 0)]]
+    s = build_stream(T1, 1 << 20)
+    got, _ = gpu_decode(s)
+    assert got.tobytes() == py_decode(T1)
+
+
+def test_empty_and_tiny():
+    for n in (0, 1, 15, 16, 17):
+        raw = np.arange(n, dtype=np.uint8)
+        comp = oracle.encode(raw, block_size=16)
+        got, _ = gpu_decode(comp)
+        assert got.tobytes() == raw.tobytes()
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5, 7, 8, 9, 15, 16, 17, 31, 32, 33, 100])
+@pytest.mark.parametrize("n", [5, 31, 32, 33, 1000, 65535])
+def test_periodic_overlap(k, n):
+    """Self-overlapping copies = periodic replication (Q3), short (one thread) and long (one warp)."""
+    pat = bytes((65 + i) % 251 for i in range(k))
+    for lead in (b"", b"xy", b"0123456789abcde"):                               # vary destination alignment
+        blocks = [[(lead + pat, n, len(lead))]]
+        s = build_stream(blocks, 1 << 17)
+        got, _ = gpu_decode(s)
+        exp = lead + (pat * (n // k + 2))[:k + n]
+        assert got.tobytes() == exp
+
+
+def test_long_copies_all_alignments():
+    """Non-overlapping long matches and long literal runs at every (src, dst) alignment mod 16."""
+    rng = np.random.default_rng(3)
+    base = rng.integers(0, 256, 4096, dtype=np.uint8).tobytes()
+    seqs = [(base, 0, 0)]
+    for sa in range(16):
+        for da in range(0, 16, 3):
+            lit = rng.integers(0, 256, 17 + da, dtype=np.uint8).tobytes()
+            seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
+    blocks = [seqs]
+    s = build_stream(blocks, 1 << 20)
+    got, _ = gpu_decode(s)
+    assert got.tobytes() == py_decode(blocks)
+
+
+@pytest.mark.parametrize("bs,nb,seed", [(16, 9, 0), (64, 37, 1), (4096, 5, 2), (1 << 16, 3, 3)])
+def test_fuzz_streams(bs, nb, seed):
+    """Encoder-free fuzz: random valid streams, arbitrary depths (deep chains), random overlaps."""
+    rng = np.random.default_rng(200 + seed)
+    for it in range(6):
+        blocks = random_blocks(rng, bs, nb, max_len=40 if bs < 4096 else 300, max_lit=12 if bs < 4096 else 40)
+        s = build_stream(blocks, bs, min_match=1)
+        exp = py_decode(blocks)
+        for strat in STRATS:
+            got, _ = gpu_decode(s, strat)
+            assert got.tobytes() == exp, (bs, nb, seed, it, strat)
+
+
+# ---------------------------------------------------------------- oracle-encoded workloads
+CASES = [("markov", 1 << 20, dict(block_size=1 << 18)),
+         ("markov", (1 << 20) + 4321, dict(block_size=1 << 16, flatten=False)),           # deep chains: hundreds of waves
+         ("markov", 1 << 20, dict(block_size=1 << 18, depth_limit=2)),
+         ("text", 3 << 20, dict()),
+         ("text", 3 << 20, dict(depth_limit=4)),
+         ("fastq", (3 << 20) + 77, dict()),
+         ("stress", 6 << 20, dict()),
+         ("stress", 4 << 20, dict(flatten=False)),
+         ("stress", 4 << 20, dict(depth_limit=1))]
+
+
+@pytest.mark.parametrize("kind,n,kw", CASES)
+def test_workload_parity(kind, n, kw):
+    raw = workloads.generate(kind, n, 260604268)
+    comp = oracle.encode(raw, **kw)
+    assert_parity(comp, raw)
+
+
+def test_config0_synth4m():
+    """BASELINE config 0 at full size: 4 blocks of 1 MB, flatten on, no depth limit."""
+    raw = workloads.config_bytes("synth4m")
+    comp = oracle.encode(raw)
+    assert_parity(comp, raw)
+
+
+def test_deeper_than_smem_bins():
+    """max_depth + 1 > 4096 takes the global-atomic bucketing path."""
+    n = 6000
+    blocks = [[(b"abcd", 0, 0)] + [(b"", 4, 4 * i) for i in range(n)]]
+    s = build_stream(blocks, 1 << 20)
+    got, st = gpu_decode(s, ax.WAVES_PERSISTENT)
+    assert st["max_depth"] == n and got.tobytes() == b"abcd" * (n + 1)
+
+
+def test_incompressible_and_runs():
+    rng = np.random.default_rng(5)
+    raw = rng.integers(0, 256, (2 << 20) + 5, dtype=np.uint8)
+    assert_parity(oracle.encode(raw), raw, [0])
+    raw = np.full(3 << 20, 0x41, np.uint8)
+    assert_parity(oracle.encode(raw), raw, [0])
+
+
+# ---------------------------------------------------------------- phases, reuse, faults
+def test_phases_and_replay():
+    from paper_2606_04268_b200.torch_io import Decoder
+    raw = workloads.generate("text", 2 << 20, 9)
+    comp = oracle.encode(raw, depth_limit=4)
+    for strat in STRATS:
+        d = Decoder(comp, 0, strat)
+        d.run(ax.PHASE_PRE)
+        d.run(ax.PHASE_MATCH)
+        assert np.array_equal(d.output(), raw)
+        for _ in range(3):                                 # plan + scratch reuse; MATCH alone replays on PRE's lists
+            d.out_dev.zero_()
+            d.run(ax.PHASE_ALL)
+            assert np.array_equal(d.output(), raw)
+        d.run(ax.PHASE_MATCH)
+        assert np.array_equal(d.output(), raw)
+        d.close()
+
+
+def test_decode_host_entry():
+    import torch
+    raw = workloads.generate("fastq", 2 << 20, 4)
+    comp = oracle.encode(raw)
+    p = ax.Plan(comp.ctypes.data, comp.size, 0)
+    ch = torch.from_numpy(comp).pin_memory()
+    oh = torch.zeros(p.raw_bytes, dtype=torch.uint8).pin_memory()
+    cd = torch.empty(comp.size, dtype=torch.uint8, device="cuda")
+    od = torch.empty(p.out_bytes, dtype=torch.uint8, device="cuda")
+    sc = torch.empty(p.scratch_bytes, dtype=torch.uint8, device="cuda")
+    p.decode_host(ch.data_ptr(), comp.size, oh.data_ptr(), oh.numel(), cd.data_ptr(), od.data_ptr(), od.numel(),
+                  sc.data_ptr(), sc.numel(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert p.stats(sc.data_ptr())["rc"] == 0
+    assert np.array_equal(oh.numpy(), raw)
+    p.close()
+
+
+def test_argument_errors():
+    import torch
+    raw = workloads.generate("markov", 100000, 1)
+    comp = oracle.encode(raw, block_size=1 << 16)
+    p = ax.Plan(comp.ctypes.data, comp.size, 0)
+    cd = torch.from_numpy(comp).cuda()
+    od = torch.empty(p.out_bytes + 16, dtype=torch.uint8, device="cuda")
+    sc = torch.empty(p.scratch_bytes + 16, dtype=torch.uint8, device="cuda")
+    L = ax._lib()
+    rc = lambda *a: L.aceapex_decode(p._h, *a)
+    assert rc(cd.data_ptr(), od.data_ptr(), p.out_bytes - 16, sc.data_ptr(), sc.numel(), 3, 0) == ax.E_CAPACITY
+    assert rc(cd.data_ptr(), od.data_ptr(), od.numel(), sc.data_ptr(), p.scratch_bytes - 1, 3, 0) == ax.E_CAPACITY
+    assert rc(cd.data_ptr(), od.data_ptr() + 1, od.numel() - 1, sc.data_ptr(), sc.numel(), 3, 0) == ax.E_ALIGN
+    assert rc(cd.data_ptr(), od.data_ptr(), od.numel(), sc.data_ptr(), sc.numel(), 0, 0) == ax.E_ARG
+    assert rc(None, od.data_ptr(), od.numel(), sc.data_ptr(), sc.numel(), 3, 0) == ax.E_ARG
+    p.close()
+
+
+def test_device_faults_are_flagged_not_fatal():
+    """Token-level faults: flagged through get_stats (E_STREAM), never an out-of-bounds access; the guard bytes
+    behind the output stay untouched."""
+    import torch
+    from paper_2606_04268_b200.torch_io import Decoder
+    good = [[(b"abcdefgh", 8, 0), (b"WX", 8, 0), (b"z", 5, 26)]]
+    s = build_stream(good, 32, flags=5)
+    po = 128
+
+    def run(t, strat=0):
+        d = Decoder(t, 0, strat)
+        guard = torch.full((4096,), 0xEE, dtype=torch.uint8, device="cuda")
+        big = torch.cat([torch.zeros(d.plan.out_bytes, dtype=torch.uint8, device="cuda"), guard])
+        d.out_dev = big
+        st = None
+        d.plan.decode(d.comp_dev.data_ptr(), big.data_ptr(), d.plan.out_bytes, d.scratch.data_ptr(), d.scratch.numel(), 3,
+                      torch.cuda.current_stream().cuda_stream)
+        st = d.stats(check=False)
+        assert bool((big[d.plan.out_bytes:] == 0xEE).all())
+        d.close()
+        return st
+
+    def mut(off, vals):
+        t = s.copy()
+        t[off:off + len(vals)] = np.frombuffer(bytes(vals), np.uint8)
+        return t
+    assert run(s)["rc"] == 0
+    for strat in STRATS:
+        st = run(mut(po, [9]), strat)                         # cmd[0] 8 -> 9: block no longer sums
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_BLOCK_SUM and st["fault_block"] == 0
+        st = run(mut(po + 48 + 4, [200]), strat)              # off[1] >= mdst
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_SOURCE
+        st = run(mut(po + 32 + 2, [0]), strat)                # dep[1] = 0 on a match
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
+        st = run(mut(po + 32 + 2, [9]), strat)                # dep[1] > max_depth
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
+        st = run(mut(po + 16 + 2, [200, 200]), strat)         # len[1] huge: would run past the block
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_BLOCK_SUM
+    two = build_stream([[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]], 32)   # depths 1,2,1
+    t = two.copy()
+    t[po + 32 + 2] = 1                                        # dep[1] 2 -> 1: counts disagree with the histogram
+    st = run(t)
+    assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
+
+
+@pytest.mark.full
+@pytest.mark.skipif(not os.environ.get("ACEAPEX_FULL"), reason="full-size configs need minutes of CPU encode; set ACEAPEX_FULL=1")
+@pytest.mark.parametrize("name,kw", [("text256m", dict()), ("fastq1g", dict()), ("text1g_d4", dict(depth_limit=4))])
+def test_full_size_configs(name, kw):
+    """BASELINE configs at full size, in bench.py's launch configuration: GPU bytes == generator bytes (which the
+    oracle round trip pins), plus sampled windows against the oracle's sequential decode of the same stream."""
+    from bench import load_workload
+    raw, comp = load_workload(name)
+    got, st = gpu_decode(comp)
+    assert np.array_equal(got, raw)
+    want = oracle.decode(comp, threads=os.cpu_count() or 1)
+    rng = np.random.default_rng(0)
+    for o in rng.integers(0, raw.size - 4096, 256):
+        assert np.array_equal(got[o:o + 4096], want[o:o + 4096])
