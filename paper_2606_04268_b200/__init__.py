@@ -117,8 +117,8 @@ class Plan:
 
     def decode(self, comp_dev: int, out_dev: int, out_capacity: int, scratch_dev: int, scratch_bytes: int,
                phases: int = PHASE_ALL, stream: int = 0):
-        _check(self._L.aceapex_decode(self._h, comp_dev, out_dev, out_capacity, scratch_dev, scratch_bytes, phases,
-                                      stream), "decode")
+        rc = self._L.aceapex_decode(self._h, comp_dev, out_dev, out_capacity, scratch_dev, scratch_bytes, phases, stream)
+        _check(rc, "decode" if rc != E_CUDA else f"decode (cudaError {self._L.aceapex_last_cuda_error(self._h)})")
 
     def decode_host(self, comp_host: int, comp_bytes: int, out_host: int, out_host_capacity: int, comp_dev: int,
                     out_dev: int, out_capacity: int, scratch_dev: int, scratch_bytes: int, stream: int = 0):

@@ -40,6 +40,7 @@ struct aceapex_plan_s {
     uint32_t last_launches; int last_strategy;
     int last_cuda;
     cudaStream_t last_stream;
+    cudaStream_t capture_stream = nullptr;
     std::vector<GraphSlot> graphs;
 };
 
@@ -240,11 +241,15 @@ extern "C" int aceapex_decode(aceapex_plan_t* p, const void* comp_dev, void* out
             p->last_launches = g.n_launches;
             return ACEAPEX_OK;
         }
+    // Capture on a private stream (the caller's may be the legacy default stream, which cannot be captured);
+    // capturing records the launches without running them, the instantiated graph then runs on the caller's stream.
     cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr; uint32_t nl = 0;
-    e = cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal);
+    e = cudaSuccess;
+    if (!p->capture_stream) e = cudaStreamCreateWithFlags(&p->capture_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamBeginCapture(p->capture_stream, cudaStreamCaptureModeThreadLocal);
     if (e == cudaSuccess) {
-        cudaError_t e2 = enqueue(p, P, phases, ACEAPEX_WAVES_LAUNCH, st, &nl);
-        e = cudaStreamEndCapture(st, &graph);
+        cudaError_t e2 = enqueue(p, P, phases, ACEAPEX_WAVES_LAUNCH, p->capture_stream, &nl);
+        e = cudaStreamEndCapture(p->capture_stream, &graph);
         if (e2 != cudaSuccess) e = e2;
     }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
@@ -306,5 +311,6 @@ extern "C" int64_t aceapex_depth_hist(const aceapex_plan_t* p, uint64_t* n_match
 extern "C" void aceapex_free(aceapex_plan_t* p) {
     if (!p) return;
     for (GraphSlot& g : p->graphs) cudaGraphExecDestroy(g.exec);
+    if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     delete p;
 }
