@@ -15,6 +15,11 @@ cudaError_t pre_configure();
 size_t pre_smem_bytes();
 int pre_max_ctas_per_sm();
 int match_max_ctas_per_sm();
+cudaError_t waves_configure();
+cudaError_t fused_configure();
+int fused_max_ctas_per_sm();
+void launch_fused(const Params& P, int grid, cudaStream_t st);
+void launch_check_cursors(const Params& P, cudaStream_t st);
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
 }  // namespace ax
@@ -33,9 +38,9 @@ struct aceapex_plan_s {
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
     uint32_t n_tiles;
     // device facts
-    int device, n_sm, pre_grid, match_ctas_per_sm;
+    int device, n_sm, pre_grid, match_ctas_per_sm, fused_grid;
     // scratch layout (byte offsets)
-    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_dst, o_off, o_len, scratch_bytes;
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_prog, o_front, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
     uint32_t last_launches; int last_strategy;
     int last_cuda;
@@ -73,8 +78,9 @@ static int choose_strategy(const aceapex_plan_t* p) {
         if (!strcmp(e, "launch")) return ACEAPEX_WAVES_LAUNCH;
         if (!strcmp(e, "graph")) return ACEAPEX_WAVES_GRAPH;
         if (!strcmp(e, "persistent")) return ACEAPEX_WAVES_PERSISTENT;
+        if (!strcmp(e, "fused") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_FUSED;
     }
-    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
+    return p->max_depth <= FUSED_MAX_DEPTH ? ACEAPEX_WAVES_FUSED : ACEAPEX_WAVES_PERSISTENT;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -128,10 +134,13 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = cudaSetDevice(device);
         if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, device);
         if (ce == cudaSuccess) ce = pre_configure();
+        if (ce == cudaSuccess) ce = waves_configure();
+        if (ce == cudaSuccess) ce = fused_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
         int pre_occ = pre_max_ctas_per_sm(); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
+        { int fo = fused_max_ctas_per_sm(); if (fo < 1) fo = 1; p->fused_grid = p->n_sm * fo; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
         if (cur >= 0 && cur != device) cudaSetDevice(cur);
         // scratch layout
@@ -141,6 +150,8 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_cursor = o; o += up256(4ull * (p->max_depth + 2));
         p->o_blocks = o; o += up256(sizeof(BlockDesc) * (size_t)nb);
         p->o_tiles = o; o += up256(8ull * p->n_tiles);
+        p->o_prog = o; o += up256(4ull * p->n_tiles);
+        p->o_front = o; o += up256(4ull * (FUSED_MAX_DEPTH + 2));
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
@@ -160,7 +171,8 @@ extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p-
 extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
 
 extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
-    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PERSISTENT) return ACEAPEX_E_ARG;
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_FUSED) return ACEAPEX_E_ARG;
+    if (s == ACEAPEX_WAVES_FUSED && p->max_depth > FUSED_MAX_DEPTH) return ACEAPEX_E_ARG;
     p->strategy_forced = s;
     return ACEAPEX_OK;
 }
@@ -177,6 +189,8 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
+    P.prog = reinterpret_cast<uint32_t*>(s + p->o_prog);
+    P.front = reinterpret_cast<uint32_t*>(s + p->o_front);
     P.raw_size = p->raw_size; P.block_size = p->block_size; P.n_blocks = p->n_blocks; P.n_tiles = p->n_tiles;
     P.max_depth = p->max_depth; P.min_match = p->min_match; P.n_match = (uint32_t)p->n_match;
     return P;
@@ -186,6 +200,14 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
 static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, int strategy, cudaStream_t st, uint32_t* n_launch) {
     uint32_t n = 0;
     if (p->n_blocks == 0) { *n_launch = 0; return cudaSuccess; }
+    if (strategy == ACEAPEX_WAVES_FUSED && phases == ACEAPEX_PHASE_ALL) {
+        launch_index(P, p->n_sm, st);
+        launch_fused(P, p->fused_grid, st);
+        launch_check_cursors(P, st);
+        *n_launch = 1 + (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
+        return cudaGetLastError();
+    }
+    if (strategy == ACEAPEX_WAVES_FUSED) strategy = p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;   // PRE / MATCH alone: list path
     if (phases & ACEAPEX_PHASE_PRE) {
         launch_index(P, p->n_sm, st); ++n;
         launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
@@ -199,7 +221,7 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
             ++n;
         } else {
             for (uint32_t d = 1; d <= p->max_depth; ++d) {
-                cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], p->n_sm * p->match_ctas_per_sm * 4, st);
+                cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], p->n_sm * p->match_ctas_per_sm, st);
                 if (e != cudaSuccess) return e;
                 if (p->hist_cnt[d]) ++n;
             }

@@ -20,8 +20,10 @@ constexpr int TILE = PRE_THREADS * PRE_ITEMS;      // 2048
 constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in shared memory; deeper streams use global atomics
 
 // ---- match kernel
-constexpr int MATCH_THREADS = 256;
-constexpr uint32_t SHORT_MAX = 32;                 // matches up to this length are copied by one thread
+constexpr int MATCH_THREADS = 256;                 // k_wave (one launch per depth)
+constexpr int PERSIST_THREADS = 1024;              // k_waves_persistent: one CTA per SM
+constexpr uint32_t SHORT_MAX = 32;
+constexpr uint32_t FUSED_MAX_DEPTH = 16;           // the fused tile kernel handles streams up to this depth                 // matches up to this length are copied by one thread
 
 // Per-block descriptor written by k_index (step a1).  Stream addresses are byte offsets from comp base.
 struct BlockDesc {
@@ -55,6 +57,8 @@ struct Params {
     uint32_t* wl_dst;                              // [n_match] match destination (absolute)
     uint32_t* wl_off;                              // [n_match] match source (absolute)
     uint16_t* wl_len;                              // [n_match]
+    uint32_t* prog;                                // [n_tiles] fused kernel: phases completed per tile
+    uint32_t* front;                               // [FUSED_MAX_DEPTH + 2] fused kernel: leading tiles with prog >= p
     uint64_t raw_size;
     uint32_t block_size, n_blocks, n_tiles, max_depth, min_match, n_match;
 };
@@ -86,40 +90,27 @@ __device__ __forceinline__ uint4 shift16(uint4 a, uint4 b, uint32_t sh) {
 
 // ---- warp-cooperative copy of n bytes, source and destination ranges disjoint.
 // dst: 16-byte aligned vector stores on the body, byte stores on head/tail; never stores outside [dst, dst+n).
-// src: whole aligned 16-byte words are loaded (bypassing L1: the data may have been written by another SM
-// earlier in the same kernel), so up to 15 bytes beyond either end of the source range may be READ.
+// src: whole aligned 16-byte words are loaded (plain L1-cached loads: callers order them after the producing wave
+// by a kernel boundary or an acquiring grid barrier), so up to 15 bytes beyond either end of the source may be READ.
 __device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t lane) {
     uint32_t h = (uint32_t)(-(intptr_t)dst) & 15u;
     if (h > n) h = n;
-    if (lane < h) dst[lane] = __ldcg(src + lane);
+    if (lane < h) dst[lane] = src[lane];
     dst += h; src += h; n -= h;
     const uint32_t nvec = n >> 4;
     const uint32_t sh = (uint32_t)((uintptr_t)src & 15u);
     const uint4* s16 = reinterpret_cast<const uint4*>(src - sh);
     uint4* d16 = reinterpret_cast<uint4*>(dst);
     if (sh == 0) {
-        for (uint32_t v = lane; v < nvec; v += 32) d16[v] = __ldcg(s16 + v);
+        for (uint32_t v = lane; v < nvec; v += 32) d16[v] = s16[v];
     } else {
         for (uint32_t v = lane; v < nvec; v += 32) {
-            const uint4 a = __ldcg(s16 + v), b = __ldcg(s16 + v + 1);
+            const uint4 a = s16[v], b = s16[v + 1];
             d16[v] = shift16(a, b, sh);
         }
     }
     const uint32_t t = n & 15u, tb = nvec << 4;
-    if (lane < t) dst[tb + lane] = __ldcg(src + tb + lane);
-}
-
-// ---- warp-cooperative periodic fill: dst[i] = src[i mod period], i < n (overlapping match, Q3).
-// Reads only the first `period` source bytes, which exist before the match starts.
-__device__ __forceinline__ void warp_fill_periodic(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t period,
-                                                   uint32_t lane) {
-    uint32_t j = lane % period;
-    const uint32_t step = 32 % period;
-    for (uint32_t i = lane; i < n; i += 32) {
-        dst[i] = __ldcg(src + j);
-        j += step;
-        if (j >= period) j -= period;
-    }
+    if (lane < t) dst[tb + lane] = src[tb + lane];
 }
 
 }  // namespace ax

@@ -1,0 +1,124 @@
+// copy.cuh — byte-copy primitives of the match copy (step a6) shared by the wave kernel (k_match.cu) and the fused
+// tile kernel (k_fused.cu).  All take explicit destination / source pointers (generic: global or shared memory).
+// Contract of every routine: it stores exactly the bytes [d, d+len) and nothing else; it loads only from
+// [s - 15, s + min(len, dist) + 15] rounded to aligned words — never a byte the match itself produces, unless the
+// routine says so (warp_match's doubling, which requires source and destination to live in the same memory).
+#pragma once
+#include "common.cuh"
+
+namespace ax {
+
+// ---- 128-bit value in two registers: byte i of the value is byte i of lo (i < 8) or byte i-8 of hi
+struct V16 { unsigned long long lo, hi; };
+
+__device__ __forceinline__ V16 shr_bytes(V16 v, uint32_t nb) {          // v >> 8*nb, nb in 0..15
+    if (nb >= 8) { v.lo = v.hi >> ((nb - 8) * 8); v.hi = 0; }
+    else if (nb) { v.lo = (v.lo >> (nb * 8)) | (v.hi << (64 - nb * 8)); v.hi >>= nb * 8; }
+    return v;
+}
+__device__ __forceinline__ V16 shl_bytes(V16 v, uint32_t nb) {          // v << 8*nb, nb in 1..15
+    if (nb >= 8) { v.hi = v.lo << ((nb - 8) * 8); v.lo = 0; }
+    else { v.hi = (v.hi << (nb * 8)) | (v.lo >> (64 - nb * 8)); v.lo <<= nb * 8; }
+    return v;
+}
+
+// The first min(n, 16) bytes at s as a register value; reads whole aligned 8-byte words, so up to 7 bytes before
+// s and after the range are loaded and discarded (output buffers are padded to 16 bytes).
+__device__ __forceinline__ V16 load16(const uint8_t* s, uint32_t n) {
+    const uint32_t sb = (uint32_t)((uintptr_t)s & 7u), need = sb + (n > 16 ? 16 : n);
+    const unsigned long long* p = reinterpret_cast<const unsigned long long*>(s - sb);
+    const unsigned long long w0 = p[0];
+    const unsigned long long w1 = need > 8 ? p[1] : 0ull;
+    const unsigned long long w2 = need > 16 ? p[2] : 0ull;
+    V16 v;
+    if (sb) { const uint32_t sh = sb * 8; v.lo = (w0 >> sh) | (w1 << (64 - sh)); v.hi = (w1 >> sh) | (w2 << (64 - sh)); }
+    else { v.lo = w0; v.hi = w1; }
+    return v;
+}
+
+// Store the first n (<= 16) bytes of v at q with naturally aligned 1/2/4/8-byte stores, nothing outside [q, q+n).
+__device__ __forceinline__ void store16(uint8_t* q, V16 v, uint32_t n) {
+    if (((uintptr_t)q & 1) && n >= 1) { *q = (uint8_t)v.lo; v = shr_bytes(v, 1); q += 1; n -= 1; }
+    if (((uintptr_t)q & 2) && n >= 2) { *reinterpret_cast<uint16_t*>(q) = (uint16_t)v.lo; v = shr_bytes(v, 2); q += 2; n -= 2; }
+    if (((uintptr_t)q & 4) && n >= 4) { *reinterpret_cast<uint32_t*>(q) = (uint32_t)v.lo; v = shr_bytes(v, 4); q += 4; n -= 4; }
+    if (n >= 8) { *reinterpret_cast<unsigned long long*>(q) = v.lo; v.lo = v.hi; q += 8; n -= 8; }
+    if (n >= 8) { *reinterpret_cast<unsigned long long*>(q) = v.lo; return; }
+    if (n & 4) { *reinterpret_cast<uint32_t*>(q) = (uint32_t)v.lo; v.lo >>= 32; q += 4; }
+    if (n & 2) { *reinterpret_cast<uint16_t*>(q) = (uint16_t)v.lo; v.lo >>= 16; q += 2; }
+    if (n & 1) *q = (uint8_t)v.lo;
+}
+
+// v holds `period` (1..15) valid bytes: extend it periodically to 16 bytes.
+__device__ __forceinline__ V16 extend_period(V16 v, uint32_t period) {
+    if (period < 8) { v.lo &= (1ull << (period * 8)) - 1ull; v.hi = 0; }
+    else if (period == 8) v.hi = 0;
+    else v.hi &= (1ull << ((period - 8) * 8)) - 1ull;
+    for (uint32_t d = period; d < 16; d <<= 1) { const V16 s = shl_bytes(v, d); v.lo |= s.lo; v.hi |= s.hi; }
+    return v;
+}
+
+// v = 16 bytes of a pattern whose period divides c (c <= 16): the 16 bytes starting at phase ph (< period).
+// (v >> ph) supplies bytes 0 .. 15-ph; (v << (c-ph)) supplies bytes c-ph .. 15; where both do, they agree.
+__device__ __forceinline__ V16 pattern_at(V16 v, uint32_t c, uint32_t ph) {
+    V16 r = shr_bytes(v, ph);
+    if (c - ph < 16) { const V16 l = shl_bytes(v, c - ph); r.lo |= l.lo; r.hi |= l.hi; }
+    return r;
+}
+
+// One thread copies one short match (len <= SHORT_MAX = 32) through registers: d[i] = s[i mod dist], dist = d - s
+// in the output's coordinates (passed in, because d and s may point into different memories).  Loads only bytes of
+// [s, s + min(len, dist)).
+__device__ __forceinline__ void thread_copy(uint8_t* d, const uint8_t* s, uint32_t len, uint32_t dist) {
+    if (dist >= len) {                                   // no overlap
+        store16(d, load16(s, len), len > 16 ? 16 : len);
+        if (len > 16) store16(d + 16, load16(s + 16, len - 16), len - 16);
+    } else if (dist >= 16) {                             // overlap, 16 <= period < len <= 32: [0,dist) then [dist,len) = s[0 ..)
+        store16(d, load16(s, 16), 16);
+        if (dist > 16) store16(d + 16, load16(s + 16, dist - 16), dist - 16);
+        store16(d + dist, load16(s, len - dist), len - dist);
+    } else {                                             // period < 16: replicate it in registers; every chunk of
+        const V16 v = extend_period(load16(s, dist), dist);   // c = floor(16/period)*period bytes starts at phase 0
+        const uint32_t c = (16u / dist) * dist;
+        for (uint32_t done = 0; done < len; done += c) store16(d + done, v, len - done < c ? len - done : c);
+    }
+}
+
+// One warp copies one long match.  same_mem: d and s address the same memory (so that d - s == dist as pointers and
+// a step may read what an earlier step stored); otherwise only [s, s+dist) is ever read.
+__device__ __forceinline__ void warp_match(uint8_t* d, const uint8_t* s, uint32_t len, uint32_t dist, bool same_mem, uint32_t lane) {
+    if (dist >= len) { warp_copy(d, s, len, lane); return; }
+    if (dist >= 16) {
+        if (same_mem) {
+            // after `done` bytes the range [s, s+dist+done) is valid periodic data, so the copied span doubles every
+            // step; __syncwarp orders one step's stores before the next step's loads
+            uint32_t done = 0;
+            while (done < len) {
+                const uint32_t n = len - done < dist + done ? len - done : dist + done;
+                warp_copy(d + done, s, n, lane);
+                done += n;
+                __syncwarp();
+            }
+        } else {
+            for (uint32_t done = 0; done < len; done += dist) warp_copy(d + done, s, len - done < dist ? len - done : dist, lane);
+        }
+        return;
+    }
+    // period < 16: the 16 bytes at byte x of the match are the periodic pattern at phase x mod period
+    const V16 v = extend_period(load16(s, dist), dist);
+    const uint32_t c = (16u / dist) * dist;                          // 9..16, a multiple of the period
+    uint32_t n = len;
+    uint32_t h = (uint32_t)(-(intptr_t)d) & 15u;
+    if (h > n) h = n;
+    if (lane == 0 && h) store16(d, v, h);
+    d += h; n -= h;
+    const uint32_t nvec = n >> 4;
+    uint4* d16 = reinterpret_cast<uint4*>(d);
+    for (uint32_t w = lane; w < nvec; w += 32) {
+        const V16 r = pattern_at(v, c, (h + 16u * w) % dist);
+        d16[w] = make_uint4((uint32_t)r.lo, (uint32_t)(r.lo >> 32), (uint32_t)r.hi, (uint32_t)(r.hi >> 32));
+    }
+    const uint32_t t = n & 15u;
+    if (lane == 31 && t) store16(d + 16u * nvec, pattern_at(v, c, (h + 16u * nvec) % dist), t);
+}
+
+}  // namespace ax

@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
     __shared__ uint32_t s_warp[33];
     if (blockIdx.x != 0) {   // the other CTAs clear the decoupled look-back words of k_pre
         const uint32_t n = P.n_tiles, stride = (gridDim.x - 1) * IDX_THREADS;
-        for (uint32_t i = (blockIdx.x - 1) * IDX_THREADS + threadIdx.x; i < n; i += stride) P.tile_state[i] = 0ull;
+        for (uint32_t i = (blockIdx.x - 1) * IDX_THREADS + threadIdx.x; i < n; i += stride) { P.tile_state[i] = 0ull; P.prog[i] = 0u; }
         return;
     }
     const uint8_t* dir = P.comp + HDR_BYTES;
@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
         P.status->fault_flags = 0; P.status->fault_block = 0xFFFFFFFFu; P.status->match_src_bytes = 0ull;
         P.status->ticket = 0; P.status->n_match_seen = 0; P.status->barrier = 0;
     }
+    if (threadIdx.x < FUSED_MAX_DEPTH + 2) P.front[threadIdx.x] = 0u;
     // ---- block descriptors + tile_base = exclusive prefix of ceil(n_seq / TILE)
     uint32_t carry = 0;
     for (uint32_t b0 = 0; b0 < P.n_blocks; b0 += IDX_THREADS) {

@@ -2,106 +2,221 @@
 // level-k tokens are processed in parallel"; §7.1: "within each level, tokens are independent").
 // Wave d copies, for every match of depth d, len bytes out[off ..) -> out[mdst ..); a source that overlaps
 // its destination (mdst - off < len) is the periodic extension of out[off .. mdst) (Q3).
+//
+// Work assignment: the measured length mix is 98 % <= 16 bytes on the text and FASTQ
+// workloads, so one THREAD copies one short match (len <= SHORT_MAX) through registers — the source is read as
+// two or three aligned 8-byte words and funnel-shifted, the destination is written with the widest naturally
+// aligned stores that stay inside the match — and one WARP copies one long match with 16-byte vector stores.
 // Two ways of sequencing the waves (a7): one launch per depth (k_wave; plain or replayed from a CUDA graph,
 // PAPER.md:97), or one cooperative kernel with a grid barrier between depths (k_waves_persistent).
-// Every source byte of wave d was written by an earlier wave / the literal scatter; loads of `out` bypass L1
-// (ld.global.cg) because in the persistent kernel they may have been written by another SM in this launch.
-// Stores never touch a byte outside the match's own output range.
+// Every source byte of wave d was written by an earlier wave or by the literal scatter.  Loads of `out` are plain
+// (L1-cached) loads: a kernel boundary, or the acquire fence of the grid barrier, invalidates L1 before any wave
+// reads what an earlier wave wrote on another SM.  Stores never touch a byte outside the match's own range.
 #include "common.cuh"
+#include "copy.cuh"
 
 namespace ax {
 
-// One thread copies one short match (len <= SHORT_MAX).
-__device__ __forceinline__ void thread_copy(uint8_t* out, uint32_t mdst, uint32_t off, uint32_t len) {
-    const uint32_t dist = mdst - off;
-    const uint8_t* s = out + off;
-    uint8_t* d = out + mdst;
-    uint32_t j = 0;
-    for (uint32_t i = 0; i < len; ++i) {
-        d[i] = __ldcg(s + j);
-        if (++j == dist) j = 0;
+// The matches [first, last) of one wave list: one thread per short match, one warp per long match.  Each warp
+// takes WAVE_UNROLL x 32 consecutive entries per step; all entry loads, then all source loads, are issued before
+// the first store so that several DRAM/L2 round trips overlap per thread.
+
+struct Ent { uint32_t mdst, off, len; };
+
+__device__ __forceinline__ Ent load_ent(const Params& P, uint32_t i, uint32_t last) {
+    Ent e; e.mdst = 0; e.off = 0; e.len = 0;
+    if (i < last) { e.mdst = P.wl_dst[i]; e.off = P.wl_off[i]; e.len = P.wl_len[i]; }
+    return e;
+}
+
+__device__ __forceinline__ bool is_simple(const Ent& e) {   // one 16-byte register copy, no overlap handling needed
+    return e.len != 0 && e.len <= 16 && (e.mdst - e.off) >= e.len;
+}
+
+__device__ __forceinline__ void long_matches(uint8_t* out, const Ent& e, uint32_t lane) {
+    uint32_t longm = __ballot_sync(0xFFFFFFFFu, e.len > SHORT_MAX);
+    while (longm) {
+        const int sl = __ffs(longm) - 1; longm &= longm - 1;
+        const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, e.mdst, sl), o2 = __shfl_sync(0xFFFFFFFFu, e.off, sl),
+                       n2 = __shfl_sync(0xFFFFFFFFu, e.len, sl);
+        warp_match(out + d2, out + o2, n2, d2 - o2, true, lane);
     }
 }
 
-// The matches [first, last) of one wave list, 32 per warp step.
-__device__ __forceinline__ void wave_body(const Params& P, uint32_t first, uint32_t last, uint32_t warp_global,
-                                          uint32_t n_warps, uint32_t lane) {
-    for (uint32_t base = first + warp_global * 32u; base < last; base += n_warps * 32u) {
-        const uint32_t i = base + lane;
-        uint32_t mdst = 0, off = 0, len = 0;
-        if (i < last) { mdst = P.wl_dst[i]; off = P.wl_off[i]; len = P.wl_len[i]; }
-        if (len != 0 && len <= SHORT_MAX) thread_copy(P.out, mdst, off, len);
-        uint32_t longm = __ballot_sync(0xFFFFFFFFu, len > SHORT_MAX);
-        while (longm) {
-            const int sl = __ffs(longm) - 1; longm &= longm - 1;
-            const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, mdst, sl), o2 = __shfl_sync(0xFFFFFFFFu, off, sl),
-                           n2 = __shfl_sync(0xFFFFFFFFu, len, sl);
-            const uint32_t dist = d2 - o2;
-            if (dist >= n2) warp_copy(P.out + d2, P.out + o2, n2, lane);
-            else warp_fill_periodic(P.out + d2, P.out + o2, n2, dist, lane);
-        }
+// e[] already loaded: copy them (warp-converged call).  Phase A issues every source load of the U entries in
+// straight-line predicated code (no branch between them) so that U round trips to L2 overlap per thread; phase B
+// shifts and stores.  "Simple" = no overlap handling and the source fits two aligned 8-byte words.
+template <int U>
+__device__ __forceinline__ void copy_ents(uint8_t* out, const Ent (&e)[U], uint32_t lane) {
+    uint4 wa[U], wb[U];
+    bool simple[U];
+#pragma unroll
+    for (int k = 0; k < U; ++k) {
+        const uint32_t sb = e[k].off & 15u;
+        simple[k] = e[k].len != 0 && e[k].len <= 16 && (e[k].mdst - e[k].off) >= e[k].len;
+        const uint4* p = reinterpret_cast<const uint4*>(out + (simple[k] ? (e[k].off & ~15u) : 0u));
+        wa[k] = p[0];                                              // out has >= 16 bytes: offset 0 is always readable
+        wb[k] = make_uint4(0u, 0u, 0u, 0u);
+        if (simple[k] && sb + e[k].len > 16) wb[k] = p[1];
     }
+#pragma unroll
+    for (int k = 0; k < U; ++k) {
+        if (simple[k]) {
+            const uint32_t sb = e[k].off & 15u, s = (sb & 7u) * 8;
+            const unsigned long long a0 = (unsigned long long)wa[k].x | ((unsigned long long)wa[k].y << 32),
+                                     a1 = (unsigned long long)wa[k].z | ((unsigned long long)wa[k].w << 32),
+                                     b0 = (unsigned long long)wb[k].x | ((unsigned long long)wb[k].y << 32),
+                                     b1 = (unsigned long long)wb[k].z | ((unsigned long long)wb[k].w << 32);
+            const unsigned long long x0 = sb < 8 ? a0 : a1, x1 = sb < 8 ? a1 : b0, x2 = sb < 8 ? b0 : b1;
+            V16 v;
+            if (s) { v.lo = (x0 >> s) | (x1 << (64 - s)); v.hi = (x1 >> s) | (x2 << (64 - s)); } else { v.lo = x0; v.hi = x1; }
+            store16(out + e[k].mdst, v, e[k].len);
+        } else if (e[k].len != 0 && e[k].len <= SHORT_MAX) thread_copy(out + e[k].mdst, out + e[k].off, e[k].len, e[k].mdst - e[k].off);
+    }
+#pragma unroll
+    for (int k = 0; k < U; ++k) long_matches(out, e[k], lane);
 }
 
-__device__ __forceinline__ void wave_bounds(const Params& P, uint32_t d, uint32_t& first, uint32_t& last) {
-    first = P.wave_off[d];
-    const uint32_t cap = P.wave_off[d + 1], cur = P.cursor[d];   // entries actually written by PRE: [first, min(cur, cap))
-    last = cur < cap ? cur : cap;
-}
-
-__global__ void __launch_bounds__(MATCH_THREADS) k_wave(Params P, uint32_t depth) {
-    uint32_t first, last;
-    wave_bounds(P, depth, first, last);
-    const uint32_t wpb = MATCH_THREADS / 32;
-    wave_body(P, first, last, blockIdx.x * wpb + (threadIdx.x >> 5), gridDim.x * wpb, threadIdx.x & 31);
-}
-
-// Grid barrier: monotone counter in scratch (zeroed by the host before the launch); cooperative launch
-// guarantees all CTAs are resident.  Release: fence before the arrive; acquire: fence after the spin.
+// Grid barrier: monotone counter in scratch (zeroed by the host before the launch); the cooperative launch
+// guarantees all CTAs are resident.  One release-reduction per CTA, a relaxed spin, one acquire fence (which
+// also invalidates L1 — SASS: CCTL.IVALL).  Measured on B200, 148 CTAs: 1.26 us.
 __device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t target) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(ctr, 1u);
+        asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(ctr), "r"(1u) : "memory");
         uint32_t v;
-        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory"); } while (v < target);
-        __threadfence();
+        do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory"); } while (v < target);
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
     }
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(MATCH_THREADS) k_waves_persistent(Params P, uint32_t d_first, uint32_t d_last) {
-    const uint32_t wpb = MATCH_THREADS / 32;
-    const uint32_t warp_global = blockIdx.x * wpb + (threadIdx.x >> 5), n_warps = gridDim.x * wpb, lane = threadIdx.x & 31;
+// ---- the wave kernel: a software pipeline over "pieces" of the wave lists
+// CTA c owns the slice [first + c*per, first + (c+1)*per) of every wave's list, cut into pieces of <= PIECE
+// entries.  Stage k+2's entries travel global -> shared with cp.async (no registers, no stall) while stage k+1's
+// source lines are prefetched into L2 and stage k is copied, so after a grid barrier only L2-hit source loads and
+// the stores themselves are on the critical path (DRAM latency on B200 is ~1 us; a wave costs ~3 of them if the
+// entry load, the source load and the barrier are taken one after the other).
+constexpr uint32_t PIECE = 4096;                         // entries per piece (4 per thread)
+constexpr uint32_t NSTAGE = 3;
+constexpr uint32_t OFF_WIN = 1024;                       // wave_off window kept in shared memory
+
+struct WaveSmem {
+    uint32_t dst[NSTAGE][PIECE];
+    uint32_t off[NSTAGE][PIECE];
+    uint16_t len[NSTAGE][PIECE + 8];
+    uint32_t woff[OFF_WIN + 2];
+};
+
+struct Piece { uint32_t a, n, depth; bool first_of_wave, valid; };
+
+__device__ __forceinline__ void cp_async4(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+
+__global__ void __launch_bounds__(PERSIST_THREADS, 1) k_waves(Params P, uint32_t d_first, uint32_t d_last) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    WaveSmem& S = *reinterpret_cast<WaveSmem*>(smem_raw);
+    if (P.status->fault_flags & F_DEPTH) return;          // wave lists incomplete (k_check_cursors): copy nothing.
+                                                          // Uniform over the grid: the flag is final before this kernel starts.
+    const uint32_t tid = threadIdx.x, lane = tid & 31, nct = gridDim.x, cta = blockIdx.x;
+    // ---- piece iterator (identical in every thread of the CTA)
+    uint32_t it_d = d_first, it_pos = 0, it_hi = 0, win0 = d_first;
+    bool it_new = true;                                   // the next piece opens wave it_d
+    auto load_window = [&]() {
+        for (uint32_t i = tid; i < OFF_WIN + 2 && win0 + i <= P.max_depth + 1; i += PERSIST_THREADS) S.woff[i] = P.wave_off[win0 + i];
+        __syncthreads();
+    };
+    load_window();
+    auto next_piece = [&]() -> Piece {
+        Piece pc; pc.valid = false; pc.a = 0; pc.n = 0; pc.depth = 0; pc.first_of_wave = false;
+        if (it_d > d_last) return pc;
+        if (it_new) {
+            if (it_d - win0 >= OFF_WIN) { __syncthreads(); win0 = it_d; load_window(); }
+            const uint32_t first = S.woff[it_d - win0], cnt = S.woff[it_d - win0 + 1] - first;
+            const uint32_t per = (cnt + nct - 1) / nct;
+            const uint32_t lo = cta * per < cnt ? cta * per : cnt, hi = (cta + 1) * per < cnt ? (cta + 1) * per : cnt;
+            it_pos = first + lo; it_hi = first + hi;
+        }
+        pc.valid = true; pc.depth = it_d; pc.first_of_wave = it_new;
+        pc.a = it_pos; pc.n = it_hi - it_pos < PIECE ? it_hi - it_pos : PIECE;
+        it_pos += pc.n; it_new = false;
+        if (it_pos >= it_hi) { ++it_d; it_new = true; }
+        return pc;
+    };
+    auto issue = [&](const Piece& pc, uint32_t st) {
+        if (pc.valid) {
+            for (uint32_t i = tid; i < pc.n; i += PERSIST_THREADS) {
+                cp_async4(&S.dst[st][i], P.wl_dst + pc.a + i);
+                cp_async4(&S.off[st][i], P.wl_off + pc.a + i);
+            }
+            // lengths are u16: copy the 4-byte words that cover [a, a+n); S.len[st][i - (a & ~1)] holds entry i
+            const uint32_t a2 = pc.a & ~1u, nw = (pc.a + pc.n - a2 + 1) >> 1;
+            for (uint32_t w = tid; w < nw; w += PERSIST_THREADS) cp_async4(&S.len[st][2 * w], P.wl_len + a2 + 2 * w);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    Piece pc[NSTAGE];
+    pc[0] = next_piece(); issue(pc[0], 0);
+    pc[1] = next_piece(); issue(pc[1], 1);
+    asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece 0 landed (this thread's part)
+    __syncthreads();
     uint32_t epoch = 0;
-    for (uint32_t d = d_first; d <= d_last; ++d) {
-        uint32_t first, last;
-        wave_bounds(P, d, first, last);
-        wave_body(P, first, last, warp_global, n_warps, lane);
-        if (d != d_last) { epoch += gridDim.x; grid_barrier(&P.status->barrier, epoch); }
+    for (uint32_t k = 0; pc[k % NSTAGE].valid; ++k) {
+        const uint32_t s0 = k % NSTAGE, s1 = (k + 1) % NSTAGE, s2 = (k + 2) % NSTAGE;
+        pc[s2] = next_piece(); issue(pc[s2], s2);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed
+        __syncthreads();
+        if (pc[s1].valid && pc[s1].first_of_wave) {        // pull the source lines of the next wave's first piece into L2
+            const uint32_t sh = pc[s1].a & 1u;
+            for (uint32_t i = tid; i < pc[s1].n; i += PERSIST_THREADS)
+                if (S.len[s1][i + sh]) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.off[s1][i]));
+        }
+        const Piece cur = pc[s0];
+        if (cur.first_of_wave && cur.depth != d_first) { epoch += nct; grid_barrier(&P.status->barrier, epoch); }
+        {
+            const uint32_t sh = cur.a & 1u;
+            Ent e[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const uint32_t i = tid + r * PERSIST_THREADS;
+                e[r].mdst = 0; e[r].off = 0; e[r].len = 0;
+                if (i < cur.n) { e[r].mdst = S.dst[s0][i]; e[r].off = S.off[s0][i]; e[r].len = S.len[s0][i + sh]; }
+            }
+            copy_ents<4>(P.out, e, lane);
+        }
+        __syncthreads();                                   // stage s0 is free for piece k+3
     }
+}
+
+size_t waves_smem_bytes() { return sizeof(WaveSmem); }
+
+cudaError_t waves_configure() {
+    return cudaFuncSetAttribute(k_waves, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WaveSmem));
 }
 
 int match_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_waves_persistent, MATCH_THREADS, 0) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_waves, PERSIST_THREADS, sizeof(WaveSmem)) != cudaSuccess) return 0;
     return n;
 }
 
+// One wave as an ordinary launch (strategies LAUNCH and GRAPH): no barrier is executed when d_first == d_last.
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st) {
     if (n_entries == 0) return cudaSuccess;
-    uint32_t grid = (n_entries + MATCH_THREADS - 1) / MATCH_THREADS;      // one entry per thread ...
-    if (grid > (uint32_t)max_grid) grid = max_grid;                       // ... capped; the warp loop strides
-    k_wave<<<grid, MATCH_THREADS, 0, st>>>(P, depth);
+    uint32_t grid = (n_entries + PERSIST_THREADS - 1) / PERSIST_THREADS;
+    if (grid > (uint32_t)max_grid) grid = max_grid;
+    k_waves<<<grid, PERSIST_THREADS, sizeof(WaveSmem), st>>>(P, depth, depth);
     return cudaGetLastError();
 }
 
+// All waves d_first .. d_last in one cooperative launch (strategy PERSISTENT).
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(&P.status->barrier, 0, sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     Params p = P;
     void* args[] = {&p, &d_first, &d_last};
-    return cudaLaunchCooperativeKernel((const void*)k_waves_persistent, dim3(grid), dim3(MATCH_THREADS), args, 0, st);
+    return cudaLaunchCooperativeKernel((const void*)k_waves, dim3(grid), dim3(PERSIST_THREADS), args, sizeof(WaveSmem), st);
 }
 
 }  // namespace ax

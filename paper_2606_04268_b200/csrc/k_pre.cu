@@ -199,6 +199,10 @@ __global__ void k_check_cursors(Params P) {
     if (d <= P.max_depth && P.cursor[d] != P.wave_off[d + 1]) raise_fault(P.status, F_DEPTH, 0xFFFFFFFEu);
 }
 
+void launch_check_cursors(const Params& P, cudaStream_t st) {
+    if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
+}
+
 size_t pre_smem_bytes() { return sizeof(PreSmem); }
 
 cudaError_t pre_configure() {

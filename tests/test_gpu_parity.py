@@ -12,7 +12,13 @@ from streams import build_stream, py_decode, py_depths, random_blocks
 
 pytestmark = pytest.mark.gpu
 
-STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]
+STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]       # the wave-list path, three ways of sequencing
+ALL_STRATS = STRATS + [ax.WAVES_FUSED]                                # + the fused tile kernel (max_depth <= 16 only)
+
+
+def fused_ok(comp):
+    """The fused tile kernel accepts streams of max_depth <= 16 (header offset 40)."""
+    return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) <= 16
 
 
 def gpu_decode(comp, strategy=0, check=True):
@@ -30,6 +36,8 @@ def gpu_decode(comp, strategy=0, check=True):
 def assert_parity(comp, raw=None, strategies=STRATS):
     want = oracle.decode(comp)
     rep = oracle.validate(comp)
+    if strategies is STRATS and fused_ok(comp):
+        strategies = ALL_STRATS
     for s in strategies:
         got, st = gpu_decode(comp, s)
         assert got.size == want.size
@@ -74,9 +82,10 @@ def test_periodic_overlap(k, n):
     for lead in (b"", b"xy", b"0123456789abcde"):                               # vary destination alignment
         blocks = [[(lead + pat, n, len(lead))]]
         s = build_stream(blocks, 1 << 17)
-        got, _ = gpu_decode(s)
         exp = lead + (pat * (n // k + 2))[:k + n]
-        assert got.tobytes() == exp
+        for strat in (ax.WAVES_FUSED, ax.WAVES_PERSISTENT):
+            got, _ = gpu_decode(s, strat)
+            assert got.tobytes() == exp, strat
 
 
 def test_long_copies_all_alignments():
@@ -90,8 +99,9 @@ def test_long_copies_all_alignments():
             seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
     blocks = [seqs]
     s = build_stream(blocks, 1 << 20)
-    got, _ = gpu_decode(s)
-    assert got.tobytes() == py_decode(blocks)
+    for strat in (ax.WAVES_FUSED, ax.WAVES_LAUNCH):
+        got, _ = gpu_decode(s, strat)
+        assert got.tobytes() == py_decode(blocks), strat
 
 
 @pytest.mark.parametrize("bs,nb,seed", [(16, 9, 0), (64, 37, 1), (4096, 5, 2), (1 << 16, 3, 3)])
@@ -102,7 +112,7 @@ def test_fuzz_streams(bs, nb, seed):
         blocks = random_blocks(rng, bs, nb, max_len=40 if bs < 4096 else 300, max_lit=12 if bs < 4096 else 40)
         s = build_stream(blocks, bs, min_match=1)
         exp = py_decode(blocks)
-        for strat in STRATS:
+        for strat in (ALL_STRATS if fused_ok(s) else STRATS):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, it, strat)
 
@@ -155,7 +165,7 @@ def test_phases_and_replay():
     from paper_2606_04268_b200.torch_io import Decoder
     raw = workloads.generate("text", 2 << 20, 9)
     comp = oracle.encode(raw, depth_limit=4)
-    for strat in STRATS:
+    for strat in ALL_STRATS:
         d = Decoder(comp, 0, strat)
         d.run(ax.PHASE_PRE)
         d.run(ax.PHASE_MATCH)
@@ -232,7 +242,7 @@ def test_device_faults_are_flagged_not_fatal():
         t[off:off + len(vals)] = np.frombuffer(bytes(vals), np.uint8)
         return t
     assert run(s)["rc"] == 0
-    for strat in STRATS:
+    for strat in ALL_STRATS:
         st = run(mut(po, [9]), strat)                         # cmd[0] 8 -> 9: block no longer sums
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_BLOCK_SUM and st["fault_block"] == 0
         st = run(mut(po + 48 + 4, [200]), strat)              # off[1] >= mdst
@@ -246,8 +256,9 @@ def test_device_faults_are_flagged_not_fatal():
     two = build_stream([[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]], 32)   # depths 1,2,1
     t = two.copy()
     t[po + 32 + 2] = 1                                        # dep[1] 2 -> 1: counts disagree with the histogram
-    st = run(t)
-    assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
+    for strat in [0] + ALL_STRATS:
+        st = run(t, strat)
+        assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
 
 
 @pytest.mark.full
@@ -264,3 +275,32 @@ def test_full_size_configs(name, kw):
     rng = np.random.default_rng(0)
     for o in rng.integers(0, raw.size - 4096, 256):
         assert np.array_equal(got[o:o + 4096], want[o:o + 4096])
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_fuzz_shallow_streams_fused(seed):
+    """Encoder-free fuzz restricted to depth <= 16 (sources drawn from literal bytes or shallow matches), so that
+    the fused tile kernel sees random overlaps, tile-straddling sources and multi-tile blocks."""
+    rng = np.random.default_rng(900 + seed)
+    for bs, nb in ((64, 40), (4096, 6), (1 << 16, 3), (1 << 18, 2)):
+        blocks = random_blocks(rng, bs, nb, max_len=60 if bs < 4096 else 400, max_lit=12 if bs < 4096 else 60, p_match=0.7)
+        deps, bd = py_depths(blocks, bs)
+        # cut chains: a match deeper than 12 is replaced by literals of the same bytes
+        exp = py_decode(blocks)
+        pos, nblocks = 0, []
+        for blk, dd in zip(blocks, deps):
+            nb_ = []
+            for (lit, mlen, off), d in zip(blk, dd):
+                pos += len(lit)
+                if mlen and d > 12:
+                    nb_.append((lit + exp[pos:pos + mlen], 0, 0))
+                else:
+                    nb_.append((lit, mlen, off))
+                pos += mlen
+            nblocks.append(nb_)
+        assert py_decode(nblocks) == exp
+        s = build_stream(nblocks, bs, min_match=1)
+        assert fused_ok(s)
+        for strat in (ax.WAVES_FUSED, ax.WAVES_PERSISTENT):
+            got, _ = gpu_decode(s, strat)
+            assert got.tobytes() == exp, (bs, nb, seed, strat)
