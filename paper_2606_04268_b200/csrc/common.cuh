@@ -57,6 +57,8 @@ struct Params {
     uint32_t* wl_dst;                              // [n_match] match destination (absolute)
     uint32_t* wl_off;                              // [n_match] match source (absolute)
     uint16_t* wl_len;                              // [n_match]
+    uint32_t* seg_start;                           // [n_tiles * (FUSED_MAX_DEPTH+1)] shallow streams: tile's slice start per depth
+    uint32_t* seg_cnt;                             // [n_tiles * (FUSED_MAX_DEPTH+1)] ... and its length
     uint32_t* prog;                                // [n_tiles] fused kernel: phases completed per tile
     uint32_t* front;                               // [FUSED_MAX_DEPTH + 2] fused kernel: leading tiles with prog >= p
     uint64_t raw_size;

@@ -48,6 +48,11 @@ struct FusedSmem {
     unsigned long long depth_mask;                   // bit d: the tile has a match of depth d (d <= 63)
     uint32_t tile;
     uint32_t cnt[FUSED_MAX_DEPTH + 3];               // matches per depth in this tile (checked against the header histogram)
+    uint32_t dstart[FUSED_MAX_DEPTH + 3];            // depth-sorted entry list: depth d occupies [dstart[d], dstart[d+1])
+    uint16_t wcnt[PRE_THREADS / 32][FUSED_MAX_DEPTH + 2];   // per warp, per depth: matches, then exclusive base in the list
+    uint32_t e_dst[TILE];                            // the tile's matches sorted by depth
+    uint32_t e_off[TILE];
+    uint16_t e_len[TILE];
     __align__(16) uint8_t ob[OB_BYTES + 32];
 };
 
@@ -67,12 +72,18 @@ __device__ __forceinline__ void wait_ready(const Params& P, uint32_t tile, uint3
         f = __shfl_sync(0xFFFFFFFFu, f, 0);
         const uint32_t f0 = f;
         while (f < tile) {
-            const uint32_t idx = f + lane;
-            const uint32_t v = idx < tile ? f_ld32(P.prog + idx) : 0xFFFFFFFFu;
-            const uint32_t notok = __ballot_sync(0xFFFFFFFFu, v < p);
-            const uint32_t lead = notok ? (uint32_t)__ffs(notok) - 1u : 32u;
+            // 128 flags per round trip (4 per lane); lead = number of leading flags that are >= p
+            uint32_t v[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { const uint32_t idx = f + 32u * r + lane; v[r] = idx < tile ? f_ld32(P.prog + idx) : 0xFFFFFFFFu; }
+            uint32_t lead = 0;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const uint32_t notok = __ballot_sync(0xFFFFFFFFu, v[r] < p);
+                if (lead == 32u * r) lead += notok ? (uint32_t)__ffs(notok) - 1u : 32u;
+            }
             f = f + lead < tile ? f + lead : tile;
-            if (lead == 0) __nanosleep(64);
+            if (lead == 0) __nanosleep(32);
         }
         if (lane == 0) {
             asm volatile("fence.acq_rel.gpu;" ::: "memory");
@@ -222,7 +233,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_fused(Params P) {
             c[k] = mdst;                                     // reuse c[] as the match destination
             if (!m) { l[k] = 0; dp[k] = 0; }
         }
-        // depths present in the tile (max_depth <= 63 on this path)
+        // ---- sort the tile's matches by depth into shared memory (a5, per tile): warp-ballot ranks
         {
             unsigned long long dm = 0ull;
 #pragma unroll
@@ -230,42 +241,92 @@ __global__ void __launch_bounds__(PRE_THREADS, 3) k_fused(Params P) {
 #pragma unroll
             for (int d = 16; d; d >>= 1) dm |= __shfl_xor_sync(0xFFFFFFFFu, dm, d);
             if (lane == 0 && dm) atomicOr(&S.depth_mask, dm);
+            for (uint32_t d = 1; d <= P.max_depth; ++d) {
+                uint32_t n = 0;
+                if ((dm >> d) & 1ull) {
+#pragma unroll
+                    for (int k = 0; k < PRE_ITEMS; ++k) n += __popc(__ballot_sync(0xFFFFFFFFu, l[k] != 0 && dp[k] == d));
+                }
+                if (lane == 0) S.wcnt[warp][d] = (uint16_t)n;
+            }
+            __syncthreads();
+            if (tid == 0) {                                  // depth-major exclusive scan over (depth, warp): <= 17 x 8 adds
+                uint32_t run = 0;
+                for (uint32_t d = 1; d <= P.max_depth; ++d) {
+                    S.dstart[d] = run;
+                    for (int w = 0; w < PRE_THREADS / 32; ++w) { const uint32_t n = S.wcnt[w][d]; S.wcnt[w][d] = (uint16_t)run; run += n; }
+                    S.cnt[d] = run - S.dstart[d];
+                }
+                S.dstart[P.max_depth + 1] = run;
+            }
+            __syncthreads();
+            for (uint32_t d = 1; d <= P.max_depth; ++d) {
+                if (!((dm >> d) & 1ull)) continue;
+                uint32_t at = S.wcnt[warp][d];
+#pragma unroll
+                for (int k = 0; k < PRE_ITEMS; ++k) {
+                    const bool mine = l[k] != 0 && dp[k] == d;
+                    const uint32_t m = __ballot_sync(0xFFFFFFFFu, mine);
+                    if (mine) { const uint32_t i = at + __popc(m & ((1u << lane) - 1u)); S.e_dst[i] = c[k]; S.e_off[i] = of[k]; S.e_len[i] = (uint16_t)l[k]; }
+                    at += __popc(m);
+                }
+            }
         }
         __syncthreads();
         if (in_smem) flush_tile(P.out, S.ob - tb, t0, t1);
         publish(P.prog, tile, 1u);
         const unsigned long long dmask = S.depth_mask;
-        // per-depth match counts of the tile -> cursor[d] (k_check_cursors compares them with the header histogram)
-        for (uint32_t d = 1; d <= P.max_depth; ++d) {
-            if (!((dmask >> d) & 1ull)) continue;
-            uint32_t n = 0;
-#pragma unroll
-            for (int k = 0; k < PRE_ITEMS; ++k) n += __popc(__ballot_sync(0xFFFFFFFFu, l[k] != 0 && dp[k] == d));
-            if (lane == 0 && n) atomicAdd(&S.cnt[d], n);
-        }
-        __syncthreads();
+        // per-depth match counts -> cursor[d] (k_check_cursors compares them with the header histogram)
         if (tid >= 1 && tid <= P.max_depth && S.cnt[tid]) atomicAdd(&P.cursor[tid], S.cnt[tid]);
         // ---- phases 1 .. max_depth: matches of depth d (a6), sequenced by the progress flags (a7)
+        const uint8_t* const img = S.ob - tb;                // img + x = byte x of the output, if in_smem and x in [tb, t1)
         for (uint32_t d = 1; d <= P.max_depth; ++d) {
             if (!((dmask >> d) & 1ull)) continue;
             wait_ready(P, tile, d);
+            const uint32_t e0 = S.dstart[d], e1 = S.dstart[d + 1];
+            for (uint32_t base = e0 + warp * 64u; base < e1; base += (PRE_THREADS / 32) * 64u) {
+                uint32_t md[2], so[2], ln[2];
+                uint4 wa[2], wb[2];
+                bool simple[2];
+                const uint8_t* sp[2];
 #pragma unroll
-            for (int k = 0; k < PRE_ITEMS; ++k) {
-                const bool mine = l[k] != 0 && dp[k] == d;
-                const uint32_t dist = c[k] - of[k];
-                // a source that starts inside the tile is read from the shared image (it may never have reached
-                // global memory in this phase order only if it is this match's own output, which is in shared too)
-                const bool src_sm = in_smem && of[k] >= t0;
-                const uint8_t* sp = src_sm ? (const uint8_t*)(S.ob - tb) + of[k] : (const uint8_t*)P.out + of[k];
-                if (mine && l[k] <= SHORT_MAX) thread_copy(wbase + c[k], sp, l[k], dist);
-                uint32_t longm = __ballot_sync(0xFFFFFFFFu, mine && l[k] > SHORT_MAX);
-                while (longm) {
-                    const int sl = __ffs(longm) - 1; longm &= longm - 1;
-                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, c[k], sl), o2 = __shfl_sync(0xFFFFFFFFu, of[k], sl),
-                                   n2 = __shfl_sync(0xFFFFFFFFu, l[k], sl);
-                    const bool ssm = in_smem && o2 >= t0;
-                    const uint8_t* sp2 = ssm ? (const uint8_t*)(S.ob - tb) + o2 : (const uint8_t*)P.out + o2;
-                    warp_match(wbase + d2, sp2, n2, d2 - o2, ssm || !in_smem, lane);
+                for (int r = 0; r < 2; ++r) {
+                    const uint32_t i = base + 32u * r + lane;
+                    md[r] = 0; so[r] = 0; ln[r] = 0;
+                    if (i < e1) { md[r] = S.e_dst[i]; so[r] = S.e_off[i]; ln[r] = S.e_len[i]; }
+                    // a source that starts inside the tile is read from the shared image
+                    sp[r] = (in_smem && so[r] >= t0) ? img + so[r] : (const uint8_t*)P.out + so[r];
+                    simple[r] = ln[r] != 0 && ln[r] <= 16 && (md[r] - so[r]) >= ln[r];
+                    const uint32_t sb = so[r] & 15u;
+                    const uint4* p = reinterpret_cast<const uint4*>(sp[r] - sb);      // shared image keeps the output's alignment mod 16
+                    wa[r] = make_uint4(0u, 0u, 0u, 0u); wb[r] = wa[r];
+                    if (simple[r]) { wa[r] = p[0]; if (sb + ln[r] > 16) wb[r] = p[1]; }
+                }
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    if (simple[r]) {
+                        const uint32_t sb = so[r] & 15u, sh = (sb & 7u) * 8;
+                        const unsigned long long a0 = (unsigned long long)wa[r].x | ((unsigned long long)wa[r].y << 32),
+                                                 a1 = (unsigned long long)wa[r].z | ((unsigned long long)wa[r].w << 32),
+                                                 b0 = (unsigned long long)wb[r].x | ((unsigned long long)wb[r].y << 32),
+                                                 b1 = (unsigned long long)wb[r].z | ((unsigned long long)wb[r].w << 32);
+                        const unsigned long long x0 = sb < 8 ? a0 : a1, x1 = sb < 8 ? a1 : b0, x2 = sb < 8 ? b0 : b1;
+                        V16 v;
+                        if (sh) { v.lo = (x0 >> sh) | (x1 << (64 - sh)); v.hi = (x1 >> sh) | (x2 << (64 - sh)); } else { v.lo = x0; v.hi = x1; }
+                        store16(wbase + md[r], v, ln[r]);
+                    } else if (ln[r] != 0 && ln[r] <= SHORT_MAX) thread_copy(wbase + md[r], sp[r], ln[r], md[r] - so[r]);
+                }
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    uint32_t longm = __ballot_sync(0xFFFFFFFFu, ln[r] > SHORT_MAX);
+                    while (longm) {
+                        const int sl = __ffs(longm) - 1; longm &= longm - 1;
+                        const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, md[r], sl), o2 = __shfl_sync(0xFFFFFFFFu, so[r], sl),
+                                       n2 = __shfl_sync(0xFFFFFFFFu, ln[r], sl);
+                        const bool ssm = in_smem && o2 >= t0;
+                        const uint8_t* sp2 = ssm ? img + o2 : (const uint8_t*)P.out + o2;
+                        warp_match(wbase + d2, sp2, n2, d2 - o2, ssm || !in_smem, lane);
+                    }
                 }
             }
             __syncthreads();

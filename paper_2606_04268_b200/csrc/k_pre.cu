@@ -31,8 +31,13 @@ struct PreSmem {
     unsigned long long warp_sum[PRE_THREADS / 32];
     unsigned long long tile_prefix;      // (out << 32) | lit of everything before this tile in its block
     uint32_t tile;
+    uint32_t nloc;                       // entries placed in the tile's sorted list so far
     uint32_t cnt[SMEM_DEPTHS];           // per-depth count inside the tile
     uint32_t gbase[SMEM_DEPTHS];         // per-depth start in the wave list reserved for this tile
+    uint16_t lbase[SMEM_DEPTHS];         // per-depth start in the tile's sorted list (bins in reservation order)
+    uint32_t seg_cnt[FUSED_MAX_DEPTH + 2];   // shallow streams: this tile's matches per depth (-> P.seg_cnt)
+    uint32_t e_dst[TILE], e_off[TILE], e_g[TILE];   // the tile's matches grouped by depth; e_g = index in the wave list
+    uint16_t e_len[TILE];
 };
 
 __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
@@ -40,12 +45,14 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
     PreSmem& S = *reinterpret_cast<PreSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool smem_bins = (P.max_depth + 1) <= SMEM_DEPTHS;
+    const bool shallow = P.max_depth <= FUSED_MAX_DEPTH;     // record per-tile segments for the tiled pass kernel
     if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) S.cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
     for (;;) {
         __syncthreads();
-        if (tid == 0) S.tile = atomicAdd(&P.status->ticket, 1u);
+        if (tid == 0) { S.tile = atomicAdd(&P.status->ticket, 1u); S.nloc = 0; }
+        if (tid <= FUSED_MAX_DEPTH) S.seg_cnt[tid] = 0;
         __syncthreads();
         const uint32_t tile = S.tile;
         if (tile >= P.n_tiles) break;
@@ -173,18 +180,40 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k)
                 if (first_mask & (1u << k)) {            // reserve this tile's slice of the depth's wave list
-                    S.gbase[dp[k]] = atomicAdd(&P.cursor[dp[k]], S.cnt[dp[k]]);
+                    const uint32_t n = S.cnt[dp[k]];
+                    const uint32_t g = atomicAdd(&P.cursor[dp[k]], n);
+                    S.gbase[dp[k]] = g;
+                    S.lbase[dp[k]] = (uint16_t)atomicAdd(&S.nloc, n);
+                    if (shallow) { S.seg_cnt[dp[k]] = n; P.seg_start[(size_t)tile * (FUSED_MAX_DEPTH + 1) + dp[k]] = g; }
                     S.cnt[dp[k]] = 0;                    // bin is clean again for the next tile
                 }
             __syncthreads();
-        }
-        // ---- a5: write the wave list entries
+            if (shallow && tid >= 1 && tid <= P.max_depth) P.seg_cnt[(size_t)tile * (FUSED_MAX_DEPTH + 1) + tid] = S.seg_cnt[tid];
+            // ---- a5: group the tile's entries by depth in shared memory, then write them out in list order so
+            // that consecutive threads store consecutive list slots (coalesced runs, one per depth present)
 #pragma unroll
-        for (int k = 0; k < PRE_ITEMS; ++k) {
-            if (of[k] == 0xFFFFFFFFu) continue;
-            const uint32_t at = (smem_bins ? S.gbase[dp[k]] : 0u) + rank[k];
-            if (at >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); continue; }   // more matches than the histogram says
-            P.wl_dst[at] = c[k]; P.wl_off[at] = of[k]; P.wl_len[at] = (uint16_t)l[k];
+            for (int k = 0; k < PRE_ITEMS; ++k) {
+                if (of[k] == 0xFFFFFFFFu) continue;
+                const uint32_t i = (uint32_t)S.lbase[dp[k]] + rank[k];
+                uint32_t g = S.gbase[dp[k]] + rank[k];
+                if (g >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); g = 0xFFFFFFFFu; }   // more matches than the histogram says
+                S.e_dst[i] = c[k]; S.e_off[i] = of[k]; S.e_len[i] = (uint16_t)l[k]; S.e_g[i] = g;
+            }
+            __syncthreads();
+            const uint32_t nloc = S.nloc;
+            for (uint32_t i = tid; i < nloc; i += PRE_THREADS) {
+                const uint32_t g = S.e_g[i];
+                if (g != 0xFFFFFFFFu) { P.wl_dst[g] = S.e_dst[i]; P.wl_off[g] = S.e_off[i]; P.wl_len[g] = S.e_len[i]; }
+            }
+        } else {
+            // ---- a5 (streams deeper than the shared-memory bins): ranks came from global cursors, write directly
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) {
+                if (of[k] == 0xFFFFFFFFu) continue;
+                const uint32_t at = rank[k];
+                if (at >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); continue; }
+                P.wl_dst[at] = c[k]; P.wl_off[at] = of[k]; P.wl_len[at] = (uint16_t)l[k];
+            }
         }
     }
     // ---- M_src for the roofline report (aceapex_stats.match_src_bytes)
