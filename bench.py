@@ -131,7 +131,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    raw, comp = load_workload(args.workload, args.size_mb)
+    raw, comp = load_workload(args.workload, args.size_mb, args.enc_override)
     import oracle
     cores = host_cores()
     out = np.zeros(raw.size, dtype=np.uint8)
@@ -176,7 +176,7 @@ def run_gpu(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))   # timing plumbing only: replicas, no data-path collective
     dev = torch.device("cuda", local)
 
-    raw, comp = load_workload(args.workload, args.size_mb)
+    raw, comp = load_workload(args.workload, args.size_mb, args.enc_override)
     N = raw.size
     plan = ax.Plan(comp.ctypes.data, comp.size, local)
     if args.strategy != "auto":
@@ -302,7 +302,18 @@ def main():
     ap.add_argument("--size-mb", type=int, default=None, help="development override of the workload size")
     ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--flatten", type=int, default=None, choices=[0, 1], help="encoder override (stress sweep): chain flattening")
+    ap.add_argument("--depth-limit", type=int, default=None, help="encoder override (stress sweep): depth limit D, 0 = unlimited")
+    ap.add_argument("--prepare-only", action="store_true", help="generate + encode + cache the workload, then exit (CPU only)")
     args = ap.parse_args()
+    args.enc_override = {}
+    if args.flatten is not None:
+        args.enc_override["flatten"] = bool(args.flatten)
+    if args.depth_limit is not None:
+        args.enc_override["depth_limit"] = args.depth_limit
+    if args.prepare_only:
+        load_workload(args.workload, args.size_mb, args.enc_override)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -80,7 +80,9 @@ static int choose_strategy(const aceapex_plan_t* p) {
         if (!strcmp(e, "persistent")) return ACEAPEX_WAVES_PERSISTENT;
         if (!strcmp(e, "fused") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_FUSED;
     }
-    return p->max_depth <= FUSED_MAX_DEPTH ? ACEAPEX_WAVES_FUSED : ACEAPEX_WAVES_PERSISTENT;
+    // measured on B200: up to 8 waves one launch each beats the cooperative kernel
+    // (no barrier, full-grid launches) and the fused tile kernel (latency-bound per tile); deeper streams: persistent
+    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -213,6 +215,9 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
     }
     if (strategy == ACEAPEX_WAVES_FUSED) strategy = p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;   // PRE / MATCH alone: list path
     if (phases & ACEAPEX_PHASE_PRE) {
+        // the wave kernel OR-merges short matches into the output (copy.cuh merge16): start from zeros
+        cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);
+        if (ez != cudaSuccess) return ez;
         launch_index(P, p->n_sm, st); ++n;
         launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
         cudaError_t e = cudaGetLastError();

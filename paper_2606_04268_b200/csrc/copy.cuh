@@ -48,6 +48,23 @@ __device__ __forceinline__ void store16(uint8_t* q, V16 v, uint32_t n) {
     if (n & 1) *q = (uint8_t)v.lo;
 }
 
+// OR-merge the first n (1..16) bytes of v into ZEROED memory at q with 8-byte reductions (red.global.or.b64): one L2
+// operation per aligned word touched (1 + (n-1)/8 on average) instead of one per naturally aligned piece (~3 for a
+// 9-byte match).  Measured on B200: the L2 sustains scattered sub-word writes at a rate set by their COUNT
+// (DESIGN.md "Match copy").  Bytes outside [q, q+n) are OR-ed with zero, i.e. left as they are; every byte of the
+// output is merged exactly once, so OR equals store.  Global memory only.
+__device__ __forceinline__ void merge16(uint8_t* q, V16 v, uint32_t n) {
+    if (n < 8) { v.lo &= (1ull << (n * 8)) - 1ull; v.hi = 0; }
+    else if (n < 16) v.hi &= n == 8 ? 0ull : (1ull << ((n - 8) * 8)) - 1ull;
+    const uint32_t sb = (uint32_t)((uintptr_t)q & 7u), sh = sb * 8;
+    unsigned long long* p = reinterpret_cast<unsigned long long*>(q - sb);
+    unsigned long long w0 = v.lo, w1 = v.hi, w2 = 0ull;
+    if (sh) { w0 = v.lo << sh; w1 = (v.lo >> (64 - sh)) | (v.hi << sh); w2 = v.hi >> (64 - sh); }
+    asm volatile("red.global.or.b64 [%0], %1;" ::"l"(p), "l"(w0) : "memory");
+    if (sb + n > 8) asm volatile("red.global.or.b64 [%0], %1;" ::"l"(p + 1), "l"(w1) : "memory");
+    if (sb + n > 16) asm volatile("red.global.or.b64 [%0], %1;" ::"l"(p + 2), "l"(w2) : "memory");
+}
+
 // v holds `period` (1..15) valid bytes: extend it periodically to 16 bytes.
 __device__ __forceinline__ V16 extend_period(V16 v, uint32_t period) {
     if (period < 8) { v.lo &= (1ull << (period * 8)) - 1ull; v.hi = 0; }

@@ -14,6 +14,7 @@
 // reads what an earlier wave wrote on another SM.  Stores never touch a byte outside the match's own range.
 #include "common.cuh"
 #include "copy.cuh"
+#include <type_traits>
 
 namespace ax {
 
@@ -70,7 +71,7 @@ __device__ __forceinline__ void copy_ents(uint8_t* out, const Ent (&e)[U], uint3
             const unsigned long long x0 = sb < 8 ? a0 : a1, x1 = sb < 8 ? a1 : b0, x2 = sb < 8 ? b0 : b1;
             V16 v;
             if (s) { v.lo = (x0 >> s) | (x1 << (64 - s)); v.hi = (x1 >> s) | (x2 << (64 - s)); } else { v.lo = x0; v.hi = x1; }
-            store16(out + e[k].mdst, v, e[k].len);
+            merge16(out + e[k].mdst, v, e[k].len);
         } else if (e[k].len != 0 && e[k].len <= SHORT_MAX) thread_copy(out + e[k].mdst, out + e[k].off, e[k].len, e[k].mdst - e[k].off);
     }
 #pragma unroll
@@ -90,6 +91,17 @@ __device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t target) {
     }
     __syncthreads();
 }
+
+#ifdef AX_TRACE
+__device__ unsigned long long ax_trace[8 * 4096];
+__device__ unsigned long long ax_arr[3 * 64 * 160];
+#define TRACE_ARR(which) do { if (tid == 0 && k < 64) ax_arr[((which) * 64 + k) * 160 + cta] = gtime(); } while (0)
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TRACE(slot) do { if (cta == 0 && tid == 0 && k < 4096) ax_trace[8 * k + (slot)] = gtime(); } while (0)
+#else
+#define TRACE(slot) do {} while (0)
+#define TRACE_ARR(which) do {} while (0)
+#endif
 
 // ---- the wave kernel: a software pipeline over "pieces" of the wave lists
 // CTA c owns the slice [first + c*per, first + (c+1)*per) of every wave's list, cut into pieces of <= PIECE
@@ -144,48 +156,86 @@ __global__ void __launch_bounds__(PERSIST_THREADS, 1) k_waves(Params P, uint32_t
         if (it_pos >= it_hi) { ++it_d; it_new = true; }
         return pc;
     };
-    auto issue = [&](const Piece& pc, uint32_t st) {
+    // cp.async the piece's entries into stage st.  `wtid`/`wn`: index and number of the threads that take part (the
+    // whole CTA in the prologue; warps 1..31 in the loop, where warp 0 runs the grid barrier at the same time).
+    auto issue = [&](const Piece& pc, uint32_t st, uint32_t wtid, uint32_t wn) {
         if (pc.valid) {
-            for (uint32_t i = tid; i < pc.n; i += PERSIST_THREADS) {
+            for (uint32_t i = wtid; i < pc.n; i += wn) {
                 cp_async4(&S.dst[st][i], P.wl_dst + pc.a + i);
                 cp_async4(&S.off[st][i], P.wl_off + pc.a + i);
             }
             // lengths are u16: copy the 4-byte words that cover [a, a+n); S.len[st][i - (a & ~1)] holds entry i
             const uint32_t a2 = pc.a & ~1u, nw = (pc.a + pc.n - a2 + 1) >> 1;
-            for (uint32_t w = tid; w < nw; w += PERSIST_THREADS) cp_async4(&S.len[st][2 * w], P.wl_len + a2 + 2 * w);
+            for (uint32_t w = wtid; w < nw; w += wn) cp_async4(&S.len[st][2 * w], P.wl_len + a2 + 2 * w);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
+    // process one landed piece from stage st: one entry per thread per round, only as many rounds as it has entries
+    auto process = [&](const Piece& cur, uint32_t st) {
+        const uint32_t sh = cur.a & 1u;
+        auto run = [&](auto U_tag) {
+            constexpr int U = decltype(U_tag)::value;
+            Ent e[U];
+#pragma unroll
+            for (int r = 0; r < U; ++r) {
+                const uint32_t i = tid + r * PERSIST_THREADS;
+                e[r].mdst = 0; e[r].off = 0; e[r].len = 0;
+                if (i < cur.n) { e[r].mdst = S.dst[st][i]; e[r].off = S.off[st][i]; e[r].len = S.len[st][i + sh]; }
+            }
+            copy_ents<U>(P.out, e, lane);
+        };
+        if (cur.n <= PERSIST_THREADS) run(std::integral_constant<int, 1>{});
+        else if (cur.n <= 2 * PERSIST_THREADS) run(std::integral_constant<int, 2>{});
+        else run(std::integral_constant<int, 4>{});
+    };
     Piece pc[NSTAGE];
-    pc[0] = next_piece(); issue(pc[0], 0);
-    pc[1] = next_piece(); issue(pc[1], 1);
+    pc[0] = next_piece(); issue(pc[0], 0, tid, PERSIST_THREADS);
+    pc[1] = next_piece(); issue(pc[1], 1, tid, PERSIST_THREADS);
     asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece 0 landed (this thread's part)
     __syncthreads();
     uint32_t epoch = 0;
+    constexpr uint32_t NW = PERSIST_THREADS - 32;          // threads of warps 1..31
     for (uint32_t k = 0; pc[k % NSTAGE].valid; ++k) {
         const uint32_t s0 = k % NSTAGE, s1 = (k + 1) % NSTAGE, s2 = (k + 2) % NSTAGE;
-        pc[s2] = next_piece(); issue(pc[s2], s2);
-        asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed
-        __syncthreads();
-        if (pc[s1].valid && pc[s1].first_of_wave) {        // pull the source lines of the next wave's first piece into L2
-            const uint32_t sh = pc[s1].a & 1u;
-            for (uint32_t i = tid; i < pc[s1].n; i += PERSIST_THREADS)
-                if (S.len[s1][i + sh]) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.off[s1][i]));
-        }
         const Piece cur = pc[s0];
-        if (cur.first_of_wave && cur.depth != d_first) { epoch += nct; grid_barrier(&P.status->barrier, epoch); }
-        {
-            const uint32_t sh = cur.a & 1u;
-            Ent e[4];
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const uint32_t i = tid + r * PERSIST_THREADS;
-                e[r].mdst = 0; e[r].off = 0; e[r].len = 0;
-                if (i < cur.n) { e[r].mdst = S.dst[s0][i]; e[r].off = S.off[s0][i]; e[r].len = S.len[s0][i + sh]; }
+        TRACE(0); TRACE_ARR(0);
+        process(cur, s0);
+        TRACE(1);
+        __syncthreads();                                   // every store of this piece is issued; stage s0 is free
+        TRACE(2); TRACE_ARR(1);
+        const Piece nxt = pc[s1];
+        const bool boundary = nxt.valid && nxt.first_of_wave;   // a7: the next piece opens a new wave
+        if (boundary) epoch += nct;
+        pc[s2] = next_piece();                             // (uniform bookkeeping, all threads)
+        if (tid < 32) {
+            // warp 0: the grid barrier — arrive (release: the CTA's stores are ordered before it through the
+            // __syncthreads above), spin, acquire fence (also invalidates L1: CCTL.IVALL)
+            if (boundary && tid == 0) {
+                asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(&P.status->barrier), "r"(1u) : "memory");
+                uint32_t v;
+                do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(&P.status->barrier) : "memory"); } while (v < epoch);
+                asm volatile("fence.acq_rel.gpu;" ::: "memory");
             }
-            copy_ents<4>(P.out, e, lane);
+            asm volatile("cp.async.commit_group;" ::: "memory");   // keep every thread's group count in step
+            asm volatile("cp.async.wait_group 1;" ::: "memory");   // (warp 0 took part in the prologue's pieces 0 and 1)
+        } else {
+            // warps 1..31, meanwhile: fetch piece k+2, and once piece k+1 has landed pull the next wave's source and
+            // destination lines into L2
+            issue(pc[s2], s2, tid - 32, NW);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed (this thread's part)
+            asm volatile("bar.sync 1, %0;" ::"n"(NW) : "memory");
+            if (boundary) {
+                const uint32_t sh = nxt.a & 1u;
+                for (uint32_t i = tid - 32; i < nxt.n; i += NW)
+                    if (S.len[s1][i + sh]) {
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.off[s1][i]));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.dst[s1][i]));
+                    }
+            }
         }
-        __syncthreads();                                   // stage s0 is free for piece k+3
+        TRACE(3); TRACE_ARR(2);
+        __syncthreads();
+        TRACE(4);
     }
 }
 
@@ -220,3 +270,12 @@ cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t 
 }
 
 }  // namespace ax
+
+#ifdef AX_TRACE
+extern "C" int aceapex_trace_read(unsigned long long* host, size_t n) {   // debug builds only (-DAX_TRACE)
+    return (int)cudaMemcpyFromSymbol(host, ax::ax_trace, n * sizeof(unsigned long long));
+}
+extern "C" int aceapex_trace_read_arr(unsigned long long* host, size_t n) {
+    return (int)cudaMemcpyFromSymbol(host, ax::ax_arr, n * sizeof(unsigned long long));
+}
+#endif

@@ -30,7 +30,7 @@ __device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long 
 struct PreSmem {
     unsigned long long warp_sum[PRE_THREADS / 32];
     unsigned long long tile_prefix;      // (out << 32) | lit of everything before this tile in its block
-    uint32_t tile;
+    uint32_t next_tile;
     uint32_t nloc;                       // entries placed in the tile's sorted list so far
     uint32_t cnt[SMEM_DEPTHS];           // per-depth count inside the tile
     uint32_t gbase[SMEM_DEPTHS];         // per-depth start in the wave list reserved for this tile
@@ -49,20 +49,27 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
     if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) S.cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
+    uint32_t b = 0xFFFFFFFFu;                                // block of the previous tile of this CTA (tickets only grow)
     for (;;) {
         __syncthreads();
-        if (tid == 0) { S.tile = atomicAdd(&P.status->ticket, 1u); S.nloc = 0; }
-        if (tid <= FUSED_MAX_DEPTH) S.seg_cnt[tid] = 0;
+        // tiles are drawn only when a CTA is ready for them: a tile held back by a busy CTA would stall the
+        // look-back of every later tile of its block
+        if (tid == 0) { S.next_tile = atomicAdd(&P.status->ticket, 1u); S.nloc = 0; }
         __syncthreads();
-        const uint32_t tile = S.tile;
+        const uint32_t tile = S.next_tile;
         if (tile >= P.n_tiles) break;
-        // ---- which block: last b with tile_base[b] <= tile (blocks with n_seq = 0 own no tile)
-        uint32_t lo = 0, hi = P.n_blocks - 1;
-        while (lo < hi) {
-            const uint32_t mid = (lo + hi + 1) >> 1;
-            if (P.blocks[mid].tile_base <= tile) lo = mid; else hi = mid - 1;
+        if (tid <= FUSED_MAX_DEPTH) S.seg_cnt[tid] = 0;
+        // ---- which block: last b with tile_base[b] <= tile (binary search once, then walk forward)
+        if (b == 0xFFFFFFFFu) {
+            uint32_t lo = 0, hi = P.n_blocks - 1;
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi + 1) >> 1;
+                if (P.blocks[mid].tile_base <= tile) lo = mid; else hi = mid - 1;
+            }
+            b = lo;
+        } else {
+            while (b + 1 < P.n_blocks && P.blocks[b + 1].tile_base <= tile) ++b;
         }
-        const uint32_t b = lo;
         const BlockDesc B = P.blocks[b];
         const uint32_t t_in_blk = tile - B.tile_base;
         const uint32_t j0 = t_in_blk * TILE + tid * PRE_ITEMS;          // first sequence of this thread
@@ -107,26 +114,38 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
             if (w < (int)warp) wpre += x;
             total += x;
         }
-        if (tid == 0) {   // decoupled look-back along this block's tiles
+        if (warp == 0) {   // decoupled look-back along this block's tiles, 32 predecessors per round trip
             const uint32_t tot_o = (uint32_t)(total >> 32), tot_l = (uint32_t)total;
             uint32_t pre_o = 0, pre_l = 0;
             if (t_in_blk != 0) {
-                st_relaxed(&P.tile_state[tile], pack_state(ST_AGG, tot_o, tot_l));
-                uint32_t q = tile;
+                if (lane == 0) st_relaxed(&P.tile_state[tile], pack_state(ST_AGG, tot_o, tot_l));
+                uint32_t q0 = tile;                              // lane looks at tile q0 - 1 - lane
                 for (;;) {
-                    --q;
-                    unsigned long long s;
-                    do { s = ld_relaxed(&P.tile_state[q]); } while ((s & ST_MASK) == 0);
-                    pre_o += (uint32_t)((s >> 31) & 0x7FFFFFFFu); pre_l += (uint32_t)(s & 0x7FFFFFFFu);
+                    const bool in_blk = q0 - B.tile_base > lane;         // q0 - 1 - lane >= tile_base
+                    unsigned long long s = ST_INC;                       // before the block's first tile: inclusive 0
+                    if (in_blk) { do { s = ld_relaxed(&P.tile_state[q0 - 1 - lane]); } while ((s & ST_MASK) == 0); }
+                    const uint32_t incm = __ballot_sync(0xFFFFFFFFu, (s & ST_MASK) == ST_INC);
+                    const uint32_t upto = incm ? (uint32_t)__ffs(incm) - 1u : 31u;     // nearest inclusive predecessor
+                    uint32_t vo = lane <= upto ? (uint32_t)((s >> 31) & 0x7FFFFFFFu) : 0u;
+                    uint32_t vl = lane <= upto ? (uint32_t)(s & 0x7FFFFFFFu) : 0u;
+#pragma unroll
+                    for (int d = 16; d; d >>= 1) {
+                        vo += __shfl_xor_sync(0xFFFFFFFFu, vo, d); vl += __shfl_xor_sync(0xFFFFFFFFu, vl, d);
+                        vo = vo > SAT ? SAT : vo; vl = vl > SAT ? SAT : vl;
+                    }
+                    pre_o += vo; pre_l += vl;
                     if (pre_o > SAT) pre_o = SAT;
                     if (pre_l > SAT) pre_l = SAT;
-                    if ((s & ST_MASK) == ST_INC) break;
+                    if (incm) break;
+                    q0 -= 32;
                 }
             }
-            st_relaxed(&P.tile_state[tile], pack_state(ST_INC, pre_o + tot_o, pre_l + tot_l));
-            S.tile_prefix = ((unsigned long long)pre_o << 32) | pre_l;
-            const bool last_tile = (t_in_blk + 1) * (uint32_t)TILE >= B.n_seq;
-            if (last_tile && (pre_o + tot_o != B.raw_len || pre_l + tot_l != B.n_lit)) raise_fault(P.status, F_BLOCK_SUM, b);
+            if (lane == 0) {
+                st_relaxed(&P.tile_state[tile], pack_state(ST_INC, pre_o + tot_o, pre_l + tot_l));
+                S.tile_prefix = ((unsigned long long)pre_o << 32) | pre_l;
+                const bool last_tile = (t_in_blk + 1) * (uint32_t)TILE >= B.n_seq;
+                if (last_tile && (pre_o + tot_o != B.raw_len || pre_l + tot_l != B.n_lit)) raise_fault(P.status, F_BLOCK_SUM, b);
+            }
         }
         __syncthreads();
         const unsigned long long ex = S.tile_prefix + wpre + (inc - tsum);
