@@ -153,6 +153,32 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """Replicas only: the one cross-rank step of the bench is the MAX of the device-timed durations.
+    Works on any initialised process group (NCCL on the GPU box, gloo in the CPU tests)."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_gbs(raw_bytes: int, ms_per_step: float, world: int) -> float:
+    """Whole-job throughput of `world` independent replicas, each decoding raw_bytes per step (weak scaling)."""
+    return world * raw_bytes / (ms_per_step * 1e-3) / 1e9 if ms_per_step > 0 else 0.0
+
+
+def ncu_traffic(workload: str):
+    """DRAM bytes (read + write) of one k_waves launch from the committed ncu capture (profiles/traffic.json), else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload, {}).get("k_waves_dram_bytes")
+    except Exception:
+        return None
+
+
 def measured_peak() -> tuple[float, str]:
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -240,11 +266,7 @@ def run_gpu(args):
     e2e_tot, _ = timed(e2e, e2e_steps)
 
     def maxr(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return max_over_ranks(x, world, dev)
     tot_ms, mt_ms, pt_ms, e2e_tot = maxr(tot_ms), maxr(mt_ms), maxr(pt_ms), maxr(e2e_tot)
 
     if rank == 0:
@@ -258,7 +280,7 @@ def run_gpu(args):
         waves = [c for c in cnt[1:]]
         line = {
             "metric": "decode GB/s on 1 B200 (decompressed bytes / s, whole hot path, compressed stream resident in HBM)",
-            "value": round(world * gbs(N, ms_step), 2), "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+            "value": round(aggregate_gbs(N, ms_step, world), 2), "unit": "GB/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "u8", "data": "synthetic",
             "config": {"workload": args.workload, "raw_bytes": int(N), "comp_bytes": int(C), "n_seq": st["n_seq"], "n_match": nm,
@@ -266,7 +288,7 @@ def run_gpu(args):
                        "max_depth": st["max_depth"], "depth_limit": st["depth_limit"], "flattened": bool(st["flags"] & 1),
                        "wave_strategy": ax.STRATEGY_NAMES[st["strategy"]], "replicas": world,
                        "l2": "inputs larger than L2 (no flush)" if C + N > 256 * MiB else "small config: L2-resident, correctness only",
-                       "output_rezeroed_between_steps": True},
+                       "output_rezeroed_between_steps": True, "output_zeroing": "inside every step (library memset, timed)"},
             "match_phase": {"gbs": round(gbs(N, ms_match), 2), "ms": round(ms_match, 4), "algorithmic_bytes": int(b_match),
                             "achieved_gbs": round(gbs(b_match, ms_match), 1), "frac_of_measured_peak": round(gbs(b_match, ms_match) / peak, 4),
                             "frac_of_nominal_8000": round(gbs(b_match, ms_match) / 8000.0, 4)},
@@ -276,9 +298,10 @@ def run_gpu(args):
             "pre_phase": {"ms": round(ms_pre, 4)},
             "waves": {"n_waves": len(waves), "matches_per_wave_min_med_max": [int(min(waves)), int(sorted(waves)[len(waves) // 2]), int(max(waves))] if waves else [],
                       "depth_hist_head": [[d, int(cnt[d]), int(byt[d])] for d in range(min(len(cnt), 9))]},
-            "roofline": {"bound": "hbm", "kernel": "match waves (k_wave / k_waves_persistent, all depths of one step)",
+            "roofline": {"bound": "hbm", "kernel": "k_waves (all match waves of one step: one cooperative launch, or one launch per depth)",
                          "achieved": round(gbs(b_match, ms_match), 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                         "frac": round(gbs(b_match, ms_match) / peak, 4), "traffic": None},
+                         "frac": round(gbs(b_match, ms_match) / peak, 4), "traffic": ncu_traffic(args.workload),
+                         "algorithmic_bytes": int(b_match), "kernel_ms": round(ms_match, 4), "share_of_step": round(ms_match / ms_step, 3)},
             "e2e": {"value": round(world * gbs(N, ms_e2e), 2), "unit": "GB/s", "h2d_bytes_per_step": int(C), "d2h_bytes_per_step": int(N),
                     "ms": round(ms_e2e, 3), "steps": e2e_steps},
             "gpu_launches": int(launches_per_step * args.steps),

@@ -92,8 +92,10 @@ typedef struct {
  * Errors: E_ARG, E_MAGIC, E_VERSION, E_TRUNCATED, E_HEADER, E_NOMEM, E_CUDA.  *out is NULL on error. */
 int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out);
 
-/* Bytes the caller must provide.  aceapex_out_bytes = raw size rounded up to 16 (kernels load whole
- * aligned 16-byte words of the output; they never STORE outside [0, raw_bytes)). */
+/* Bytes the caller must provide.  aceapex_out_bytes = raw size rounded up to 16: kernels load whole aligned
+ * 16-byte words of the output and OR-merge aligned 8-byte words of it (red.or with zeros outside the token), so
+ * the padding may be read and rewritten with its own value; no byte outside [0, raw_bytes) ever CHANGES, and
+ * nothing beyond aceapex_out_bytes is touched. */
 size_t aceapex_raw_bytes(const aceapex_plan_t* p);
 size_t aceapex_out_bytes(const aceapex_plan_t* p);
 size_t aceapex_scratch_bytes(const aceapex_plan_t* p);
@@ -103,8 +105,8 @@ int aceapex_set_strategy(aceapex_plan_t* p, int strategy);
 
 /* aceapex_decode — enqueue the decode on `stream` and return without synchronising the host.
  *   comp_dev      DEVICE pointer, the same comp_bytes given to aceapex_plan, 16-byte aligned, read only.
- *   out_dev       DEVICE pointer, >= aceapex_out_bytes(p) bytes, 16-byte aligned.  Bytes [0, raw) are
- *                 written; nothing else is.
+ *   out_dev       DEVICE pointer, >= aceapex_out_bytes(p) bytes, 16-byte aligned.  PHASE_PRE first zeroes
+ *                 bytes [0, raw) (short matches are OR-merged into zeros), then bytes [0, raw) are written.
  *   scratch_dev   DEVICE pointer, >= aceapex_scratch_bytes(p) bytes, 16-byte aligned.  Contents are
  *                 undefined on entry for PHASE_PRE; PHASE_MATCH alone reuses what PRE left there.
  *   phases        ACEAPEX_PHASE_* mask.  MATCH alone requires a completed PRE on the same scratch and out

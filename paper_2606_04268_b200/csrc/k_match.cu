@@ -103,6 +103,12 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 #define TRACE_ARR(which) do {} while (0)
 #endif
 
+#ifdef AX_NO_PREFETCH
+#define AX_PREFETCH_COND && false
+#else
+#define AX_PREFETCH_COND
+#endif
+
 // ---- the wave kernel: a software pipeline over "pieces" of the wave lists
 // CTA c owns the slice [first + c*per, first + (c+1)*per) of every wave's list, cut into pieces of <= PIECE
 // entries.  Stage k+2's entries travel global -> shared with cp.async (no registers, no stall) while stage k+1's
@@ -224,7 +230,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, 1) k_waves(Params P, uint32_t
             issue(pc[s2], s2, tid - 32, NW);
             asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed (this thread's part)
             asm volatile("bar.sync 1, %0;" ::"n"(NW) : "memory");
-            if (boundary) {
+            if (boundary AX_PREFETCH_COND) {
                 const uint32_t sh = nxt.a & 1u;
                 for (uint32_t i = tid - 32; i < nxt.n; i += NW)
                     if (S.len[s1][i + sh]) {

@@ -261,12 +261,10 @@ def test_device_faults_are_flagged_not_fatal():
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
 
 
-@pytest.mark.full
-@pytest.mark.skipif(not os.environ.get("ACEAPEX_FULL"), reason="full-size configs need minutes of CPU encode; set ACEAPEX_FULL=1")
-@pytest.mark.parametrize("name,kw", [("text256m", dict()), ("fastq1g", dict()), ("text1g_d4", dict(depth_limit=4))])
-def test_full_size_configs(name, kw):
-    """BASELINE configs at full size, in bench.py's launch configuration: GPU bytes == generator bytes (which the
-    oracle round trip pins), plus sampled windows against the oracle's sequential decode of the same stream."""
+def _full_size_case(name):
+    """A BASELINE config at full size, in bench.py's launch configuration (AUTO strategy, same buffers): GPU bytes ==
+    generator bytes (which the oracle round trip pins), plus sampled windows against the oracle's decode of the same
+    stream, plus the device-side recount of M_src against the oracle validator's."""
     from bench import load_workload
     raw, comp = load_workload(name)
     got, st = gpu_decode(comp)
@@ -275,6 +273,20 @@ def test_full_size_configs(name, kw):
     rng = np.random.default_rng(0)
     for o in rng.integers(0, raw.size - 4096, 256):
         assert np.array_equal(got[o:o + 4096], want[o:o + 4096])
+    rep = oracle.validate(comp)
+    assert st["match_src_bytes"] == rep["match_src_bytes"] and st["n_match"] == rep["n_match"]
+
+
+def test_full_size_text256m():
+    """BASELINE configs[1] — the workload bench.py times by default (about a minute of CPU encode on a fresh box)."""
+    _full_size_case("text256m")
+
+
+@pytest.mark.full
+@pytest.mark.skipif(not os.environ.get("ACEAPEX_FULL"), reason="1 GiB configs need ~4 min of CPU encode each; set ACEAPEX_FULL=1")
+@pytest.mark.parametrize("name", ["fastq1g", "text1g_d4"])
+def test_full_size_1g(name):
+    _full_size_case(name)
 
 
 @pytest.mark.parametrize("seed", range(4))
