@@ -262,7 +262,7 @@ def run_gpu(args):
     torch.cuda.synchronize(dev)
     if not np.array_equal(out_host.numpy()[:N], raw):
         raise SystemExit("bench.py: host-buffer decode is not bit-exact")
-    e2e_steps = max(1, min(args.steps, 5))
+    e2e_steps = max(1, min(args.steps, 10))
     e2e_tot, _ = timed(e2e, e2e_steps)
 
     def maxr(x):
@@ -318,7 +318,7 @@ def run_gpu(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
