@@ -12,8 +12,8 @@ namespace ax {
 void launch_index(const Params& P, int n_sm, cudaStream_t st);
 void launch_pre(const Params& P, int grid, cudaStream_t st);
 cudaError_t pre_configure();
-size_t pre_smem_bytes();
-int pre_max_ctas_per_sm();
+size_t pre_smem_bytes(uint32_t max_depth);
+int pre_max_ctas_per_sm(uint32_t max_depth);
 int match_max_ctas_per_sm();
 cudaError_t waves_configure();
 cudaError_t fused_configure();
@@ -140,7 +140,7 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = fused_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
-        int pre_occ = pre_max_ctas_per_sm(); if (pre_occ < 1) pre_occ = 1;
+        int pre_occ = pre_max_ctas_per_sm(p->max_depth); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
         { int fo = fused_max_ctas_per_sm(); if (fo < 1) fo = 1; p->fused_grid = p->n_sm * fo; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;

@@ -3,24 +3,21 @@
 // Wave d copies, for every match of depth d, len bytes out[off ..) -> out[mdst ..); a source that overlaps
 // its destination (mdst - off < len) is the periodic extension of out[off .. mdst) (Q3).
 //
-// Work assignment: the measured length mix is 98 % <= 16 bytes on the text and FASTQ
-// workloads, so one THREAD copies one short match (len <= SHORT_MAX) through registers — the source is read as
-// two or three aligned 8-byte words and funnel-shifted, the destination is written with the widest naturally
-// aligned stores that stay inside the match — and one WARP copies one long match with 16-byte vector stores.
-// Two ways of sequencing the waves (a7): one launch per depth (k_wave; plain or replayed from a CUDA graph,
-// PAPER.md:97), or one cooperative kernel with a grid barrier between depths (k_waves_persistent).
+// Work assignment: the measured length mix is 98 % <= 16 bytes on the text and FASTQ workloads, so
+// one THREAD copies one short match (len <= SHORT_MAX) through registers — the source is read as one or two
+// aligned 16-byte words and funnel-shifted, the destination is OR-merged into the zeroed output with 8-byte L2
+// reductions (copy.cuh merge16) — and one WARP copies one long match with 16-byte vector stores.
+// Sequencing (a7): k_waves runs all depths in one cooperative launch with a grid barrier between
+// waves (strategy PERSISTENT), or one depth per ordinary launch (LAUNCH; GRAPH replays those launches from a CUDA
+// graph, the paper's mechanism).
 // Every source byte of wave d was written by an earlier wave or by the literal scatter.  Loads of `out` are plain
 // (L1-cached) loads: a kernel boundary, or the acquire fence of the grid barrier, invalidates L1 before any wave
-// reads what an earlier wave wrote on another SM.  Stores never touch a byte outside the match's own range.
+// reads what an earlier wave wrote on another SM.  No store or merge changes a byte outside the match's own range.
 #include "common.cuh"
 #include "copy.cuh"
 #include <type_traits>
 
 namespace ax {
-
-// The matches [first, last) of one wave list: one thread per short match, one warp per long match.  Each warp
-// takes WAVE_UNROLL x 32 consecutive entries per step; all entry loads, then all source loads, are issued before
-// the first store so that several DRAM/L2 round trips overlap per thread.
 
 struct Ent { uint32_t mdst, off, len; };
 
@@ -46,7 +43,7 @@ __device__ __forceinline__ void long_matches(uint8_t* out, const Ent& e, uint32_
 
 // e[] already loaded: copy them (warp-converged call).  Phase A issues every source load of the U entries in
 // straight-line predicated code (no branch between them) so that U round trips to L2 overlap per thread; phase B
-// shifts and stores.  "Simple" = no overlap handling and the source fits two aligned 8-byte words.
+// shifts and merges.  "Simple" = at most 16 bytes and no overlap (two aligned 16-byte words hold the source).
 template <int U>
 __device__ __forceinline__ void copy_ents(uint8_t* out, const Ent (&e)[U], uint32_t lane) {
     uint4 wa[U], wb[U];

@@ -32,21 +32,33 @@ struct PreSmem {
     unsigned long long tile_prefix;      // (out << 32) | lit of everything before this tile in its block
     uint32_t next_tile;
     uint32_t nloc;                       // entries placed in the tile's sorted list so far
-    uint32_t cnt[SMEM_DEPTHS];           // per-depth count inside the tile
-    uint32_t gbase[SMEM_DEPTHS];         // per-depth start in the wave list reserved for this tile
-    uint16_t lbase[SMEM_DEPTHS];         // per-depth start in the tile's sorted list (bins in reservation order)
     uint32_t seg_cnt[FUSED_MAX_DEPTH + 2];   // shallow streams: this tile's matches per depth (-> P.seg_cnt)
     uint32_t e_dst[TILE], e_off[TILE], e_g[TILE];   // the tile's matches grouped by depth; e_g = index in the wave list
     uint16_t e_len[TILE];
+    // followed in dynamic shared memory by the depth bins, sized to the stream (pre_bins(max_depth) entries each):
+    //   uint32_t cnt[]    per-depth count inside the tile
+    //   uint32_t gbase[]  per-depth start in the wave list reserved for this tile
+    //   uint16_t lbase[]  per-depth start in the tile's sorted list (bins in reservation order)
 };
 
-__global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
+__host__ __device__ inline uint32_t pre_bins(uint32_t max_depth) {       // 0 = deeper than the shared-memory bins
+    return max_depth + 1 <= SMEM_DEPTHS ? ((max_depth + 1 + 7u) & ~7u) : 0u;
+}
+__host__ __device__ inline size_t pre_smem_for(uint32_t max_depth) {
+    return ((sizeof(PreSmem) + 15) & ~(size_t)15) + (size_t)pre_bins(max_depth) * 10u;
+}
+
+__global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PreSmem& S = *reinterpret_cast<PreSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const bool smem_bins = (P.max_depth + 1) <= SMEM_DEPTHS;
+    const uint32_t nbins = pre_bins(P.max_depth);
+    const bool smem_bins = nbins != 0;
+    uint32_t* const s_cnt = reinterpret_cast<uint32_t*>(smem_raw + ((sizeof(PreSmem) + 15) & ~(size_t)15));
+    uint32_t* const s_gbase = s_cnt + nbins;
+    uint16_t* const s_lbase = reinterpret_cast<uint16_t*>(s_gbase + nbins);
     const bool shallow = P.max_depth <= FUSED_MAX_DEPTH;     // record per-tile segments for the tiled pass kernel
-    if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) S.cnt[i] = 0;
+    if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) s_cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
     uint32_t b = 0xFFFFFFFFu;                                // block of the previous tile of this CTA (tickets only grow)
@@ -185,7 +197,7 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
             const int leader = __ffs(peers) - 1;
             uint32_t base = 0;
             if (m && (int)lane == leader) {
-                if (smem_bins) { base = atomicAdd(&S.cnt[key], (uint32_t)__popc(peers)); if (base == 0) first_mask |= 1u << k; }
+                if (smem_bins) { base = atomicAdd(&s_cnt[key], (uint32_t)__popc(peers)); if (base == 0) first_mask |= 1u << k; }
                 else base = atomicAdd(&P.cursor[key], (uint32_t)__popc(peers));
             }
             base = __shfl_sync(0xFFFFFFFFu, base, leader);
@@ -199,12 +211,12 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k)
                 if (first_mask & (1u << k)) {            // reserve this tile's slice of the depth's wave list
-                    const uint32_t n = S.cnt[dp[k]];
+                    const uint32_t n = s_cnt[dp[k]];
                     const uint32_t g = atomicAdd(&P.cursor[dp[k]], n);
-                    S.gbase[dp[k]] = g;
-                    S.lbase[dp[k]] = (uint16_t)atomicAdd(&S.nloc, n);
+                    s_gbase[dp[k]] = g;
+                    s_lbase[dp[k]] = (uint16_t)atomicAdd(&S.nloc, n);
                     if (shallow) { S.seg_cnt[dp[k]] = n; P.seg_start[(size_t)tile * (FUSED_MAX_DEPTH + 1) + dp[k]] = g; }
-                    S.cnt[dp[k]] = 0;                    // bin is clean again for the next tile
+                    s_cnt[dp[k]] = 0;                    // bin is clean again for the next tile
                 }
             __syncthreads();
             if (shallow && tid >= 1 && tid <= P.max_depth) P.seg_cnt[(size_t)tile * (FUSED_MAX_DEPTH + 1) + tid] = S.seg_cnt[tid];
@@ -213,8 +225,8 @@ __global__ void __launch_bounds__(PRE_THREADS) k_pre(Params P) {
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k) {
                 if (of[k] == 0xFFFFFFFFu) continue;
-                const uint32_t i = (uint32_t)S.lbase[dp[k]] + rank[k];
-                uint32_t g = S.gbase[dp[k]] + rank[k];
+                const uint32_t i = (uint32_t)s_lbase[dp[k]] + rank[k];
+                uint32_t g = s_gbase[dp[k]] + rank[k];
                 if (g >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); g = 0xFFFFFFFFu; }   // more matches than the histogram says
                 S.e_dst[i] = c[k]; S.e_off[i] = of[k]; S.e_len[i] = (uint16_t)l[k]; S.e_g[i] = g;
             }
@@ -251,20 +263,20 @@ void launch_check_cursors(const Params& P, cudaStream_t st) {
     if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
 }
 
-size_t pre_smem_bytes() { return sizeof(PreSmem); }
+size_t pre_smem_bytes(uint32_t max_depth) { return pre_smem_for(max_depth); }
 
 cudaError_t pre_configure() {
-    return cudaFuncSetAttribute(k_pre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PreSmem));
+    return cudaFuncSetAttribute(k_pre, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pre_smem_for(SMEM_DEPTHS - 1));
 }
 
-int pre_max_ctas_per_sm() {
+int pre_max_ctas_per_sm(uint32_t max_depth) {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pre, PRE_THREADS, sizeof(PreSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pre, PRE_THREADS, pre_smem_for(max_depth)) != cudaSuccess) return 0;
     return n;
 }
 
 void launch_pre(const Params& P, int grid, cudaStream_t st) {
-    if (P.n_tiles) k_pre<<<grid, PRE_THREADS, sizeof(PreSmem), st>>>(P);
+    if (P.n_tiles) k_pre<<<grid, PRE_THREADS, pre_smem_for(P.max_depth), st>>>(P);
     if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
 }
 
