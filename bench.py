@@ -206,7 +206,7 @@ def run_gpu(args):
     N = raw.size
     plan = ax.Plan(comp.ctypes.data, comp.size, local)
     if args.strategy != "auto":
-        plan.set_strategy({"launch": 1, "graph": 2, "persistent": 3}[args.strategy])
+        plan.set_strategy({"launch": 1, "graph": 2, "persistent": 3, "fused": 4, "passes": 5}[args.strategy])
     comp_host = torch.from_numpy(comp).pin_memory()
     out_host = torch.empty(max(N, 1), dtype=torch.uint8).pin_memory()
     comp_dev = comp_host.to(dev)
@@ -323,7 +323,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--size-mb", type=int, default=None, help="development override of the workload size")
-    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent"])
+    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent", "fused", "passes"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--flatten", type=int, default=None, choices=[0, 1], help="encoder override (stress sweep): chain flattening")
     ap.add_argument("--depth-limit", type=int, default=None, help="encoder override (stress sweep): depth limit D, 0 = unlimited")

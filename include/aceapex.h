@@ -54,6 +54,8 @@ enum {
     ACEAPEX_WAVES_LAUNCH = 1,     /* one kernel launch per depth on the caller's stream                */
     ACEAPEX_WAVES_GRAPH = 2,      /* the same launches replayed from a cached CUDA graph */
     ACEAPEX_WAVES_PERSISTENT = 3, /* one cooperative kernel, grid barrier between depths               */
+    ACEAPEX_WAVES_PASSES = 5,     /* shallow streams (max_depth <= 16): no wave lists; the token stream is re-parsed
+                                     by one streaming kernel per depth (k_pass), prefixes from k_tilesum         */
     ACEAPEX_WAVES_FUSED = 4       /* shallow streams (max_depth <= 16), phases == ALL only: one kernel does
                                      parse + scan + literals + all waves per tile, output assembled in shared
                                      memory, tiles ordered by progress flags; PRE / MATCH alone use the lists */

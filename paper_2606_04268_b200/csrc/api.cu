@@ -20,6 +20,10 @@ cudaError_t fused_configure();
 int fused_max_ctas_per_sm();
 void launch_fused(const Params& P, int grid, cudaStream_t st);
 void launch_check_cursors(const Params& P, cudaStream_t st);
+cudaError_t pass_configure();
+int pass_max_ctas_per_sm();
+void launch_tilesum(const Params& P, int grid, cudaStream_t st);
+void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st);
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
 }  // namespace ax
@@ -38,7 +42,7 @@ struct aceapex_plan_s {
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
     uint32_t n_tiles;
     // device facts
-    int device, n_sm, pre_grid, match_ctas_per_sm, fused_grid;
+    int device, n_sm, pre_grid, match_ctas_per_sm, fused_grid, pass_grid;
     // scratch layout (byte offsets)
     size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_prog, o_front, o_seg_start, o_seg_cnt, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
@@ -79,10 +83,11 @@ static int choose_strategy(const aceapex_plan_t* p) {
         if (!strcmp(e, "graph")) return ACEAPEX_WAVES_GRAPH;
         if (!strcmp(e, "persistent")) return ACEAPEX_WAVES_PERSISTENT;
         if (!strcmp(e, "fused") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_FUSED;
+        if (!strcmp(e, "passes") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_PASSES;
     }
-    // measured on B200: up to 8 waves one launch each beats the cooperative kernel
-    // (no barrier, full-grid launches) and the fused tile kernel (latency-bound per tile); deeper streams: persistent
-    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
+    // measured on B200: up to 8 waves the list-free pass kernels win (192 vs 152 GB/s on
+    // text1g_d4; the fused tile kernel is latency-bound per tile); deeper streams: lists + persistent wave kernel
+    return p->max_depth <= 8 ? ACEAPEX_WAVES_PASSES : ACEAPEX_WAVES_PERSISTENT;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -138,11 +143,13 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = pre_configure();
         if (ce == cudaSuccess) ce = waves_configure();
         if (ce == cudaSuccess) ce = fused_configure();
+        if (ce == cudaSuccess) ce = pass_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
         int pre_occ = pre_max_ctas_per_sm(p->max_depth); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
         { int fo = fused_max_ctas_per_sm(); if (fo < 1) fo = 1; p->fused_grid = p->n_sm * fo; }
+        { int po = pass_max_ctas_per_sm(); if (po < 1) po = 1; p->pass_grid = p->n_sm * po; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
         if (cur >= 0 && cur != device) cudaSetDevice(cur);
         // scratch layout
@@ -175,8 +182,8 @@ extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p-
 extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
 
 extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
-    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_FUSED) return ACEAPEX_E_ARG;
-    if (s == ACEAPEX_WAVES_FUSED && p->max_depth > FUSED_MAX_DEPTH) return ACEAPEX_E_ARG;
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PASSES) return ACEAPEX_E_ARG;
+    if ((s == ACEAPEX_WAVES_FUSED || s == ACEAPEX_WAVES_PASSES) && p->max_depth > FUSED_MAX_DEPTH) return ACEAPEX_E_ARG;
     p->strategy_forced = s;
     return ACEAPEX_OK;
 }
@@ -213,12 +220,28 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
         *n_launch = 1 + (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
         return cudaGetLastError();
     }
+    if (strategy == ACEAPEX_WAVES_PASSES) {
+        // shallow streams without wave lists: the stream is re-parsed by every pass (k_pass.cu)
+        if (phases & ACEAPEX_PHASE_PRE) {
+            cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);   // matches are OR-merged into zeros
+            if (ez != cudaSuccess) return ez;
+            launch_index(P, p->n_sm, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
+            launch_check_cursors(P, st);
+            n += 2 + (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
+        }
+        if (phases & ACEAPEX_PHASE_MATCH)
+            for (uint32_t d = 1; d <= p->max_depth; ++d)
+                if (p->hist_cnt[d]) { launch_pass(P, d, p->pass_grid, st); ++n; }
+        *n_launch = n;
+        return cudaGetLastError();
+    }
     if (strategy == ACEAPEX_WAVES_FUSED) strategy = p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;   // PRE / MATCH alone: list path
     if (phases & ACEAPEX_PHASE_PRE) {
         // the wave kernel OR-merges short matches into the output (copy.cuh merge16): start from zeros
         cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);
         if (ez != cudaSuccess) return ez;
         launch_index(P, p->n_sm, st); ++n;
+        launch_tilesum(P, p->n_sm * 8, st); ++n;
         launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;

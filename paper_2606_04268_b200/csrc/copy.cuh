@@ -138,4 +138,61 @@ __device__ __forceinline__ void warp_match(uint8_t* d, const uint8_t* s, uint32_
     if (lane == 31 && t) store16(d + 16u * nvec, pattern_at(v, c, (h + 16u * nvec) % dist), t);
 }
 
+// ---- one wave-list entry and the register copy of U of them (wave kernel and pass kernel)
+struct Ent { uint32_t mdst, off, len; };
+
+__device__ __forceinline__ Ent load_ent(const Params& P, uint32_t i, uint32_t last) {
+    Ent e; e.mdst = 0; e.off = 0; e.len = 0;
+    if (i < last) { e.mdst = P.wl_dst[i]; e.off = P.wl_off[i]; e.len = P.wl_len[i]; }
+    return e;
+}
+
+__device__ __forceinline__ bool is_simple(const Ent& e) {   // one 16-byte register copy, no overlap handling needed
+    return e.len != 0 && e.len <= 16 && (e.mdst - e.off) >= e.len;
+}
+
+__device__ __forceinline__ void long_matches(uint8_t* out, const Ent& e, uint32_t lane) {
+    uint32_t longm = __ballot_sync(0xFFFFFFFFu, e.len > SHORT_MAX);
+    while (longm) {
+        const int sl = __ffs(longm) - 1; longm &= longm - 1;
+        const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, e.mdst, sl), o2 = __shfl_sync(0xFFFFFFFFu, e.off, sl),
+                       n2 = __shfl_sync(0xFFFFFFFFu, e.len, sl);
+        warp_match(out + d2, out + o2, n2, d2 - o2, true, lane);
+    }
+}
+
+// e[] already loaded: copy them (warp-converged call).  Phase A issues every source load of the U entries in
+// straight-line predicated code (no branch between them) so that U round trips to L2 overlap per thread; phase B
+// shifts and merges.  "Simple" = at most 16 bytes and no overlap (two aligned 16-byte words hold the source).
+template <int U>
+__device__ __forceinline__ void copy_ents(uint8_t* out, const Ent (&e)[U], uint32_t lane) {
+    uint4 wa[U], wb[U];
+    bool simple[U];
+#pragma unroll
+    for (int k = 0; k < U; ++k) {
+        const uint32_t sb = e[k].off & 15u;
+        simple[k] = e[k].len != 0 && e[k].len <= 16 && (e[k].mdst - e[k].off) >= e[k].len;
+        const uint4* p = reinterpret_cast<const uint4*>(out + (simple[k] ? (e[k].off & ~15u) : 0u));
+        wa[k] = p[0];                                              // out has >= 16 bytes: offset 0 is always readable
+        wb[k] = make_uint4(0u, 0u, 0u, 0u);
+        if (simple[k] && sb + e[k].len > 16) wb[k] = p[1];
+    }
+#pragma unroll
+    for (int k = 0; k < U; ++k) {
+        if (simple[k]) {
+            const uint32_t sb = e[k].off & 15u, s = (sb & 7u) * 8;
+            const unsigned long long a0 = (unsigned long long)wa[k].x | ((unsigned long long)wa[k].y << 32),
+                                     a1 = (unsigned long long)wa[k].z | ((unsigned long long)wa[k].w << 32),
+                                     b0 = (unsigned long long)wb[k].x | ((unsigned long long)wb[k].y << 32),
+                                     b1 = (unsigned long long)wb[k].z | ((unsigned long long)wb[k].w << 32);
+            const unsigned long long x0 = sb < 8 ? a0 : a1, x1 = sb < 8 ? a1 : b0, x2 = sb < 8 ? b0 : b1;
+            V16 v;
+            if (s) { v.lo = (x0 >> s) | (x1 << (64 - s)); v.hi = (x1 >> s) | (x2 << (64 - s)); } else { v.lo = x0; v.hi = x1; }
+            merge16(out + e[k].mdst, v, e[k].len);
+        } else if (e[k].len != 0 && e[k].len <= SHORT_MAX) thread_copy(out + e[k].mdst, out + e[k].off, e[k].len, e[k].mdst - e[k].off);
+    }
+#pragma unroll
+    for (int k = 0; k < U; ++k) long_matches(out, e[k], lane);
+}
+
 }  // namespace ax

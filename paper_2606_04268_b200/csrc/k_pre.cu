@@ -4,33 +4,16 @@
 //       PAPER.md:53 restated as a scan; one independent scan per 1 MB block)
 //   a4  out[dst[j] .. +cmd[j]) = lit_b[lsrc[j] ..)
 //   a5  matches grouped by dep[j] into per-depth wave lists (mdst, off, len)             (§7.1)
-// One tile = 2048 consecutive sequences of one block.  CTAs take tiles in order from a ticket counter, so a
-// tile's predecessors have always started: the per-block prefix is carried by decoupled look-back.  dst[] and
-// lsrc[] are never written to memory.
+// One tile = 2048 consecutive sequences of one block.  The block-level part of the scan (the prefix of each tile
+// inside its block) is computed first by k_tilesum (k_pass.cu), so tiles are independent here: static assignment,
+// no ticket, no look-back.  dst[] and lsrc[] are never written to memory.  Used for streams deeper than 8 levels;
+// shallower ones skip the wave lists altogether (k_pass.cu).
 #include "common.cuh"
 
 namespace ax {
 
-constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_MASK = 3ull << 62;
-constexpr uint32_t SAT = 0x3FFFFFFFu;   // sums saturate here (valid streams stay <= block_size <= 2^28)
-
-__device__ __forceinline__ unsigned long long pack_state(unsigned long long flag, uint32_t so, uint32_t sl) {
-    so = so > SAT ? SAT : so; sl = sl > SAT ? SAT : sl;
-    return flag | ((unsigned long long)so << 31) | (unsigned long long)sl;
-}
-__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long* p) {
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed(unsigned long long* p, unsigned long long v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
 struct PreSmem {
     unsigned long long warp_sum[PRE_THREADS / 32];
-    unsigned long long tile_prefix;      // (out << 32) | lit of everything before this tile in its block
-    uint32_t next_tile;
     uint32_t nloc;                       // entries placed in the tile's sorted list so far
     uint32_t seg_cnt[FUSED_MAX_DEPTH + 2];   // shallow streams: this tile's matches per depth (-> P.seg_cnt)
     uint32_t e_dst[TILE], e_off[TILE], e_g[TILE];   // the tile's matches grouped by depth; e_g = index in the wave list
@@ -61,27 +44,14 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
     if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) s_cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
-    uint32_t b = 0xFFFFFFFFu;                                // block of the previous tile of this CTA (tickets only grow)
-    for (;;) {
+    // Tiles are assigned statically; the per-tile prefix inside the block and the tile -> block map come from
+    // k_tilesum (k_pass.cu), so there is no ticket, no look-back and no dependency between CTAs here.
+    for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         __syncthreads();
-        // tiles are drawn only when a CTA is ready for them: a tile held back by a busy CTA would stall the
-        // look-back of every later tile of its block
-        if (tid == 0) { S.next_tile = atomicAdd(&P.status->ticket, 1u); S.nloc = 0; }
-        __syncthreads();
-        const uint32_t tile = S.next_tile;
-        if (tile >= P.n_tiles) break;
+        if (tid == 0) S.nloc = 0;
         if (tid <= FUSED_MAX_DEPTH) S.seg_cnt[tid] = 0;
-        // ---- which block: last b with tile_base[b] <= tile (binary search once, then walk forward)
-        if (b == 0xFFFFFFFFu) {
-            uint32_t lo = 0, hi = P.n_blocks - 1;
-            while (lo < hi) {
-                const uint32_t mid = (lo + hi + 1) >> 1;
-                if (P.blocks[mid].tile_base <= tile) lo = mid; else hi = mid - 1;
-            }
-            b = lo;
-        } else {
-            while (b + 1 < P.n_blocks && P.blocks[b + 1].tile_base <= tile) ++b;
-        }
+        const uint32_t b = P.prog[tile];
+        const unsigned long long tile_prefix = P.tile_state[tile];
         const BlockDesc B = P.blocks[b];
         const uint32_t t_in_blk = tile - B.tile_base;
         const uint32_t j0 = t_in_blk * TILE + tid * PRE_ITEMS;          // first sequence of this thread
@@ -119,48 +89,13 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
         }
         if (lane == 31) S.warp_sum[warp] = inc;
         __syncthreads();
-        unsigned long long wpre = 0, total = 0;
+        unsigned long long wpre = 0;
 #pragma unroll
         for (int w = 0; w < PRE_THREADS / 32; ++w) {
             const unsigned long long x = S.warp_sum[w];
             if (w < (int)warp) wpre += x;
-            total += x;
         }
-        if (warp == 0) {   // decoupled look-back along this block's tiles, 32 predecessors per round trip
-            const uint32_t tot_o = (uint32_t)(total >> 32), tot_l = (uint32_t)total;
-            uint32_t pre_o = 0, pre_l = 0;
-            if (t_in_blk != 0) {
-                if (lane == 0) st_relaxed(&P.tile_state[tile], pack_state(ST_AGG, tot_o, tot_l));
-                uint32_t q0 = tile;                              // lane looks at tile q0 - 1 - lane
-                for (;;) {
-                    const bool in_blk = q0 - B.tile_base > lane;         // q0 - 1 - lane >= tile_base
-                    unsigned long long s = ST_INC;                       // before the block's first tile: inclusive 0
-                    if (in_blk) { do { s = ld_relaxed(&P.tile_state[q0 - 1 - lane]); } while ((s & ST_MASK) == 0); }
-                    const uint32_t incm = __ballot_sync(0xFFFFFFFFu, (s & ST_MASK) == ST_INC);
-                    const uint32_t upto = incm ? (uint32_t)__ffs(incm) - 1u : 31u;     // nearest inclusive predecessor
-                    uint32_t vo = lane <= upto ? (uint32_t)((s >> 31) & 0x7FFFFFFFu) : 0u;
-                    uint32_t vl = lane <= upto ? (uint32_t)(s & 0x7FFFFFFFu) : 0u;
-#pragma unroll
-                    for (int d = 16; d; d >>= 1) {
-                        vo += __shfl_xor_sync(0xFFFFFFFFu, vo, d); vl += __shfl_xor_sync(0xFFFFFFFFu, vl, d);
-                        vo = vo > SAT ? SAT : vo; vl = vl > SAT ? SAT : vl;
-                    }
-                    pre_o += vo; pre_l += vl;
-                    if (pre_o > SAT) pre_o = SAT;
-                    if (pre_l > SAT) pre_l = SAT;
-                    if (incm) break;
-                    q0 -= 32;
-                }
-            }
-            if (lane == 0) {
-                st_relaxed(&P.tile_state[tile], pack_state(ST_INC, pre_o + tot_o, pre_l + tot_l));
-                S.tile_prefix = ((unsigned long long)pre_o << 32) | pre_l;
-                const bool last_tile = (t_in_blk + 1) * (uint32_t)TILE >= B.n_seq;
-                if (last_tile && (pre_o + tot_o != B.raw_len || pre_l + tot_l != B.n_lit)) raise_fault(P.status, F_BLOCK_SUM, b);
-            }
-        }
-        __syncthreads();
-        const unsigned long long ex = S.tile_prefix + wpre + (inc - tsum);
+        const unsigned long long ex = tile_prefix + wpre + (inc - tsum);
         uint32_t pos = (uint32_t)(ex >> 32);                 // output offset inside the block
         uint32_t lsrc = (uint32_t)ex;                        // offset inside the block's lit[]
         const uint8_t* lit = P.comp + B.lit_off;

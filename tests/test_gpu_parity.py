@@ -13,7 +13,7 @@ from streams import build_stream, py_decode, py_depths, random_blocks
 pytestmark = pytest.mark.gpu
 
 STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]       # the wave-list path, three ways of sequencing
-ALL_STRATS = STRATS + [ax.WAVES_FUSED]                                # + the fused tile kernel (max_depth <= 16 only)
+ALL_STRATS = STRATS + [ax.WAVES_FUSED, ax.WAVES_PASSES]               # + the list-free kernels (max_depth <= 16 only)
 
 
 def fused_ok(comp):
@@ -83,7 +83,7 @@ def test_periodic_overlap(k, n):
         blocks = [[(lead + pat, n, len(lead))]]
         s = build_stream(blocks, 1 << 17)
         exp = lead + (pat * (n // k + 2))[:k + n]
-        for strat in (ax.WAVES_FUSED, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, strat
 
@@ -99,7 +99,7 @@ def test_long_copies_all_alignments():
             seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
     blocks = [seqs]
     s = build_stream(blocks, 1 << 20)
-    for strat in (ax.WAVES_FUSED, ax.WAVES_LAUNCH):
+    for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_LAUNCH):
         got, _ = gpu_decode(s, strat)
         assert got.tobytes() == py_decode(blocks), strat
 
@@ -313,6 +313,6 @@ def test_fuzz_shallow_streams_fused(seed):
         assert py_decode(nblocks) == exp
         s = build_stream(nblocks, bs, min_match=1)
         assert fused_ok(s)
-        for strat in (ax.WAVES_FUSED, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, strat)
