@@ -100,46 +100,48 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
         uint32_t lsrc = (uint32_t)ex;                        // offset inside the block's lit[]
         const uint8_t* lit = P.comp + B.lit_off;
         uint8_t* outb = P.out + B.out_base;
-        // ---- a4 literal scatter + a5 ranking, sequence by sequence (loop trip count is warp-uniform)
+        // ---- a4 literal scatter + token validation (I2); c[] becomes the match destination, of[] = 0xFFFFFFFF marks
+        // "no entry" (a valid off is < mdst <= 2^32-1)
         uint32_t rank[PRE_ITEMS];
         uint32_t first_mask = 0;                             // bit k: this thread opened depth bin dp[k] in this tile
 #pragma unroll
         for (int k = 0; k < PRE_ITEMS; ++k) {
-            bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len && (uint64_t)lsrc + c[k] <= B.n_lit;
+            const bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len && (uint64_t)lsrc + c[k] <= B.n_lit;
             if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
             const uint32_t cc = ok ? c[k] : 0;
-            // literal run: short ones by their own thread, long ones by the whole warp
-            if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }
-            uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
-            while (longm) {
-                const int src_lane = __ffs(longm) - 1; longm &= longm - 1;
-                const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, src_lane), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, src_lane),
-                               n2 = __shfl_sync(0xFFFFFFFFu, cc, src_lane);
-                warp_copy(outb + p2, lit + s2, n2, lane);
+            if (__any_sync(0xFFFFFFFFu, cc != 0)) {          // literal runs are rare on compressible data: skip as a warp
+                if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }
+                uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
+                while (longm) {                              // long runs by the whole warp
+                    const int src_lane = __ffs(longm) - 1; longm &= longm - 1;
+                    const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, src_lane), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, src_lane),
+                                   n2 = __shfl_sync(0xFFFFFFFFu, cc, src_lane);
+                    warp_copy(outb + p2, lit + s2, n2, lane);
+                }
             }
             pos += c[k]; lsrc += c[k];
-            // match: validate (I2), rank inside its depth bin
             bool m = ok && l[k] != 0;
             if (l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
+            const uint32_t mdst = (uint32_t)B.out_base + pos;
             if (m) {
-                const uint64_t mdst = B.out_base + pos;
                 if (of[k] >= mdst || l[k] < P.min_match) { raise_fault(P.status, F_SOURCE, b); m = false; }
                 else if (dp[k] == 0 || dp[k] > P.max_depth) { raise_fault(P.status, F_DEPTH, b); m = false; }
             }
-            if (m) { const uint32_t dist = (uint32_t)(B.out_base + pos - of[k]); src_bytes += l[k] < dist ? l[k] : dist; }
-            const uint32_t key = m ? dp[k] : 0u;
-            const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
-            const int leader = __ffs(peers) - 1;
-            uint32_t base = 0;
-            if (m && (int)lane == leader) {
-                if (smem_bins) { base = atomicAdd(&s_cnt[key], (uint32_t)__popc(peers)); if (base == 0) first_mask |= 1u << k; }
-                else base = atomicAdd(&P.cursor[key], (uint32_t)__popc(peers));
-            }
-            base = __shfl_sync(0xFFFFFFFFu, base, leader);
-            rank[k] = base + __popc(peers & ((1u << lane) - 1u));
-            of[k] = m ? of[k] : 0xFFFFFFFFu;                 // 0xFFFFFFFF marks "no entry" (a valid off is < mdst <= 2^32-1)
-            c[k] = (uint32_t)(B.out_base + pos);             // reuse c[] as mdst
+            if (m) { const uint32_t dist = mdst - of[k]; src_bytes += l[k] < dist ? l[k] : dist; }
+            of[k] = m ? of[k] : 0xFFFFFFFFu;
+            c[k] = mdst;
             pos += l[k];
+        }
+        // ---- a5 ranking: one shared-memory atomic per match, all eight of a thread in flight at once (this kernel
+        // serves streams of more than 8 depths, where a warp's 32 keys are mostly distinct)
+#pragma unroll
+        for (int k = 0; k < PRE_ITEMS; ++k) {
+            rank[k] = 0;
+            if (of[k] != 0xFFFFFFFFu) rank[k] = smem_bins ? atomicAdd(&s_cnt[dp[k]], 1u) : atomicAdd(&P.cursor[dp[k]], 1u);
+        }
+        if (smem_bins) {
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) if (of[k] != 0xFFFFFFFFu && rank[k] == 0) first_mask |= 1u << k;
         }
         if (smem_bins) {
             __syncthreads();
