@@ -171,10 +171,11 @@ def aggregate_gbs(raw_bytes: int, ms_per_step: float, world: int) -> float:
 
 
 def ncu_traffic(workload: str):
-    """DRAM bytes (read + write) of one k_waves launch from the committed ncu capture (profiles/traffic.json), else None."""
+    """DRAM bytes (read + write) of the match kernel(s) of one step — one k_waves launch, or the k_pass launches of
+    depths 1..D — from the committed ncu capture (profiles/traffic.json), else None."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("k_waves_dram_bytes")
+            return json.load(f).get(workload, {}).get("match_dram_bytes")
     except Exception:
         return None
 
@@ -298,7 +299,7 @@ def run_gpu(args):
             "pre_phase": {"ms": round(ms_pre, 4)},
             "waves": {"n_waves": len(waves), "matches_per_wave_min_med_max": [int(min(waves)), int(sorted(waves)[len(waves) // 2]), int(max(waves))] if waves else [],
                       "depth_hist_head": [[d, int(cnt[d]), int(byt[d])] for d in range(min(len(cnt), 9))]},
-            "roofline": {"bound": "hbm", "kernel": "k_waves (all match waves of one step: one cooperative launch, or one launch per depth)",
+            "roofline": {"bound": "hbm", "kernel": ("k_pass, depths 1..D (one streaming launch per depth)" if st["strategy"] == 5 else "k_waves (all match waves of one step: one cooperative launch, or one launch per depth)"),
                          "achieved": round(gbs(b_match, ms_match), 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                          "frac": round(gbs(b_match, ms_match) / peak, 4), "traffic": ncu_traffic(args.workload),
                          "algorithmic_bytes": int(b_match), "kernel_ms": round(ms_match, 4), "share_of_step": round(ms_match / ms_step, 3)},

@@ -85,7 +85,7 @@ static int choose_strategy(const aceapex_plan_t* p) {
         if (!strcmp(e, "fused") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_FUSED;
         if (!strcmp(e, "passes") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_PASSES;
     }
-    // measured on B200 (DESIGN.md 6.2, 6.4): up to 8 waves the list-free pass kernels win (192 vs 152 GB/s on
+    // measured on B200 (DESIGN.md 6.2, 6.3): up to 8 waves the list-free pass kernels win (192 vs 152 GB/s on
     // text1g_d4; the fused tile kernel is latency-bound per tile); deeper streams: lists + persistent wave kernel
     return p->max_depth <= 8 ? ACEAPEX_WAVES_PASSES : ACEAPEX_WAVES_PERSISTENT;
 }

@@ -1,4 +1,4 @@
-// k_pass.cu — strategy PASSES for shallow streams (max_depth <= PASS_MAX_DEPTH, e.g. the depth-limited encoder of
+// k_pass.cu — strategy PASSES for shallow streams (AUTO: max_depth <= 8; accepted up to 16; e.g. the depth-limited encoder of
 // PAPER.md:228 §7.4): no wave lists at all.  The token stream is parsed once per pass instead:
 //   k_tilesum   one CTA per 1 MB block walks the block's tiles (2048 sequences each) and writes, per tile, the
 //               exclusive prefix of (cmd+len, cmd) inside the block (a3, the block-level part of the scan) and the
@@ -6,7 +6,7 @@
 //   k_pass 0    parse (a2) + scan inside the tile (a3) + literal scatter (a4) + token validation (I2) + M_src.
 //   k_pass p    parse + scan + copy of the matches with dep == p (a6), p = 1 .. max_depth, one launch each (a7: a
 //               kernel boundary orders wave p-1 before wave p).
-// Why (DESIGN.md 6.4): with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
+// Why (DESIGN.md 6.3): with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
 // and a bucketing kernel (k_pre) whose per-tile chain of ticket -> look-back -> bin reservation runs at ~1 TB/s —
 // whereas re-reading the 10 B/sequence stream is a pure streaming read with no inter-CTA dependency: tiles are
 // assigned statically, prefixes come from k_tilesum, nothing is reserved with atomics.
