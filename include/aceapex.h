@@ -75,7 +75,7 @@ typedef struct {
     uint64_t lit_bytes;       /* Lit: literal bytes (header total_lit)                                 */
     uint64_t match_bytes;     /* M = N - Lit                                                           */
     uint64_t match_src_bytes; /* M_src = sum over matches of min(len, mdst-off); counted on the device
-                                 during PRE, 0 before the first decode                                 */
+                                 during the decode, 0 before the first one                                 */
     uint64_t n_seq;           /* sequences (header total_seq)                                          */
     uint64_t n_match;         /* matches = sum of depth histogram counts for d >= 1                    */
     uint32_t n_blocks, block_size, min_match, max_depth, depth_limit, flags;

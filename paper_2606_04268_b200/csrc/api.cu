@@ -24,6 +24,7 @@ cudaError_t pass_configure();
 int pass_max_ctas_per_sm();
 void launch_tilesum(const Params& P, int grid, cudaStream_t st);
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st);
+void launch_pass_reset(const Params& P, cudaStream_t st);
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
 }  // namespace ax
@@ -226,12 +227,14 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
             cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);   // matches are OR-merged into zeros
             if (ez != cudaSuccess) return ez;
             launch_index(P, p->n_sm, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
-            launch_check_cursors(P, st);
-            n += 2 + (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
+            n += 2 + (p->n_tiles ? 1 : 0);
         }
-        if (phases & ACEAPEX_PHASE_MATCH)
-            for (uint32_t d = 1; d <= p->max_depth; ++d)
-                if (p->hist_cnt[d]) { launch_pass(P, d, p->pass_grid, st); ++n; }
+        if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
+            // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
+            launch_pass_reset(P, st); ++n;
+            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); ++n; }
+            launch_check_cursors(P, st); ++n;
+        }
         *n_launch = n;
         return cudaGetLastError();
     }

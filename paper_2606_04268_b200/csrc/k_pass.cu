@@ -3,9 +3,10 @@
 //   k_tilesum   one CTA per 1 MB block walks the block's tiles (2048 sequences each) and writes, per tile, the
 //               exclusive prefix of (cmd+len, cmd) inside the block (a3, the block-level part of the scan) and the
 //               tile's block index; checks that the block sums to raw_len / n_lit (invariant I1).
-//   k_pass 0    parse (a2) + scan inside the tile (a3) + literal scatter (a4) + token validation (I2) + M_src.
-//   k_pass p    parse + scan + copy of the matches with dep == p (a6), p = 1 .. max_depth, one launch each (a7: a
-//               kernel boundary orders wave p-1 before wave p).
+//   k_pass 0    parse cmd[], len[] (a2) + scan inside the tile (a3) + literal scatter (a4).
+//   k_pass p    parse + scan + validation (I2), M_src and copy of the matches with dep == p (a6), p = 1 .. max_depth,
+//               one launch each (a7: a kernel boundary orders wave p-1 before wave p); a match whose
+//               dep is 0 or above max_depth is copied by no pass and shows up as a histogram mismatch (F_DEPTH).
 // Why: with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
 // and a bucketing kernel (k_pre) whose per-tile chain of ticket -> look-back -> bin reservation runs at ~1 TB/s —
 // whereas re-reading the 10 B/sequence stream is a pure streaming read with no inter-CTA dependency: tiles are
@@ -92,13 +93,15 @@ __global__ void __launch_bounds__(PRE_THREADS) k_tilesum(Params P) {
 }
 
 // ---- pass p: 0 = literals + validation, p >= 1 = matches of depth p
+template <bool LIT>   // LIT: pass 0 (literals); otherwise p >= 1
 __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PassSmem& S = *reinterpret_cast<PassSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     unsigned long long src_bytes = 0;
-    if (p != 0 && P.status->fault_flags != 0) return;                 // a faulty stream is flagged, not decoded further
-    if (p == 0 && tid <= FUSED_MAX_DEPTH) S.cnt[tid] = 0;
+    if (!LIT && P.status->fault_flags != 0) return;                 // a faulty stream is flagged, not decoded further
+    if (tid <= FUSED_MAX_DEPTH) S.cnt[tid] = 0;
+    __syncthreads();
     for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         const uint32_t b = P.prog[tile];
         const unsigned long long pre = P.tile_state[tile];
@@ -109,9 +112,12 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
         if (j0 < B.n_seq) {
             const uint4 vc = *reinterpret_cast<const uint4*>(P.comp + B.cmd_off + 2ull * j0);
             const uint4 vl = *reinterpret_cast<const uint4*>(P.comp + B.len_off + 2ull * j0);
-            const uint4 vd = *reinterpret_cast<const uint4*>(P.comp + B.dep_off + 2ull * j0);
-            const uint4 o0 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0);
-            const uint4 o1 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0 + 16);
+            uint4 vd = make_uint4(0u, 0u, 0u, 0u), o0 = vd, o1 = vd;
+            if (!LIT) {                                  // pass 0 (literals) needs neither depths nor sources
+                vd = *reinterpret_cast<const uint4*>(P.comp + B.dep_off + 2ull * j0);
+                o0 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0);
+                o1 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0 + 16);
+            }
             const uint32_t wc[4] = {vc.x, vc.y, vc.z, vc.w}, wl[4] = {vl.x, vl.y, vl.z, vl.w}, wd[4] = {vd.x, vd.y, vd.z, vd.w};
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
@@ -126,28 +132,50 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k) { c[k] = 0; l[k] = 0; dp[k] = 0; of[k] = 0; }
         }
-        // ---- a3: scan inside the tile; the block-level prefix comes from k_tilesum
-        unsigned long long tsum = 0;
+        // ---- a3: scan inside the tile; the block-level prefix comes from k_tilesum.  The literal pass scans the pair
+        // (cmd+len, cmd) packed in one u64; match passes need output positions only (32-bit shuffles)
+        uint32_t pos, lsrc = 0;
+        if (LIT) {
+            unsigned long long tsum = 0;
 #pragma unroll
-        for (int k = 0; k < PRE_ITEMS; ++k) tsum += ((unsigned long long)(c[k] + l[k]) << 32) | c[k];
-        unsigned long long inc = tsum;
+            for (int k = 0; k < PRE_ITEMS; ++k) tsum += ((unsigned long long)(c[k] + l[k]) << 32) | c[k];
+            unsigned long long inc = tsum;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-            if (lane >= d) inc += t;
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            __syncthreads();                             // previous tile's readers of warp_sum are done
+            if (lane == 31) S.warp_sum[warp] = inc;
+            __syncthreads();
+            unsigned long long wpre = 0;
+#pragma unroll
+            for (int w = 0; w < PS_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
+            const unsigned long long ex = pre + wpre + (inc - tsum);
+            pos = (uint32_t)(ex >> 32);                  // output offset inside the block
+            lsrc = (uint32_t)ex;                         // offset inside the block's lit[]
+        } else {
+            uint32_t tsum = 0;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) tsum += c[k] + l[k];
+            uint32_t inc = tsum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            __syncthreads();
+            if (lane == 31) S.warp_sum[warp] = inc;
+            __syncthreads();
+            uint32_t wpre = 0;
+#pragma unroll
+            for (int w = 0; w < PS_WARPS; ++w) if (w < (int)warp) wpre += (uint32_t)S.warp_sum[w];
+            pos = (uint32_t)(pre >> 32) + wpre + (inc - tsum);
         }
-        __syncthreads();                                 // previous tile's readers of warp_sum are done
-        if (lane == 31) S.warp_sum[warp] = inc;
-        __syncthreads();
-        unsigned long long wpre = 0;
-#pragma unroll
-        for (int w = 0; w < PS_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
-        const unsigned long long ex = pre + wpre + (inc - tsum);
-        uint32_t pos = (uint32_t)(ex >> 32);             // output offset inside the block
-        uint32_t lsrc = (uint32_t)ex;                    // offset inside the block's lit[]
         const uint32_t blk_lo = (uint32_t)B.out_base;
-        if (p == 0) {
-            // ---- a4 literal scatter, token validation (I2), M_src, per-depth counts
+        if (LIT) {
+            // ---- a4 literal scatter (token validation, M_src and the per-depth counts are taken by the pass that
+            // copies the match: pass 0 reads only cmd[], len[] and lit[])
             const uint8_t* lit = P.comp + B.lit_off;
             uint8_t* outb = P.out + B.out_base;
 #pragma unroll
@@ -163,33 +191,20 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
                                    n2 = __shfl_sync(0xFFFFFFFFu, cc, sl);
                     warp_copy(outb + p2, lit + s2, n2, lane);
                 }
-                pos += c[k]; lsrc += c[k];
-                bool m = ok && l[k] != 0;
-                if (l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
-                const uint32_t mdst = blk_lo + pos;
-                if (m) {
-                    if (of[k] >= mdst || l[k] < P.min_match) { raise_fault(P.status, F_SOURCE, b); m = false; }
-                    else if (dp[k] == 0 || dp[k] > P.max_depth) { raise_fault(P.status, F_DEPTH, b); m = false; }
-                }
-                if (m) { const uint32_t dist = mdst - of[k]; src_bytes += l[k] < dist ? l[k] : dist; }
-                pos += l[k];
-                if (!m) dp[k] = 0;
-            }
-            for (uint32_t d = 1; d <= P.max_depth; ++d) {        // histogram check (k_check_cursors)
-                uint32_t n = 0;
-#pragma unroll
-                for (int k = 0; k < PRE_ITEMS; ++k) n += __popc(__ballot_sync(0xFFFFFFFFu, dp[k] == d));
-                if (lane == 0 && n) atomicAdd(&S.cnt[d], n);
+                pos += c[k] + l[k]; lsrc += c[k];
             }
         } else {
             // ---- a6: select this pass's matches (same validity rule as pass 0), compact them per warp, copy
-            uint32_t at = 0;
+            uint32_t at = 0, sb = 0;
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k) {
                 const bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len;
                 pos += c[k];
                 const uint32_t mdst = blk_lo + pos;
-                const bool sel = ok && l[k] != 0 && dp[k] == p && of[k] < mdst && l[k] >= P.min_match;
+                bool sel = ok && l[k] != 0 && dp[k] == p;
+                if (sel && (of[k] >= mdst || l[k] < P.min_match)) { raise_fault(P.status, F_SOURCE, b); sel = false; }   // I2
+                if (p == 1 && l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
+                if (sel) { const uint32_t dist = mdst - of[k]; sb += l[k] < dist ? l[k] : dist; }
                 const uint32_t msk = __ballot_sync(0xFFFFFFFFu, sel);
                 if (sel) {
                     const uint32_t i = at + __popc(msk & ((1u << lane) - 1u));
@@ -198,6 +213,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
                 at += __popc(msk);
                 pos += l[k];
             }
+            src_bytes += sb;
+            if (lane == 0 && at) atomicAdd(&S.cnt[p], at);          // histogram check (k_check_cursors after the last pass)
             __syncwarp();
             for (uint32_t base = 0; base < at; base += 64) {
                 Ent e[2];
@@ -212,22 +229,34 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pass(Params P, uint32_t p) {
             __syncwarp();
         }
     }
-    if (p == 0) {
+    if (!LIT) {
         __syncthreads();
-        if (tid >= 1 && tid <= P.max_depth && S.cnt[tid]) atomicAdd(&P.cursor[tid], S.cnt[tid]);
+        if (tid == 0 && S.cnt[p]) atomicAdd(&P.cursor[p], S.cnt[p]);
 #pragma unroll
         for (int d = 16; d; d >>= 1) src_bytes += __shfl_xor_sync(0xFFFFFFFFu, src_bytes, d);
         if (lane == 0 && src_bytes) atomicAdd(&P.status->match_src_bytes, src_bytes);
     }
 }
 
+// Before the match passes of a step: the counters they accumulate start from the header's offsets again, so that
+// PHASE_MATCH can be replayed on its own (this is how the match phase is timed alone).
+__global__ void k_pass_reset(Params P) {
+    const uint32_t d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d == 0) P.status->match_src_bytes = 0ull;
+    if (d >= 1 && d <= P.max_depth) P.cursor[d] = P.wave_off[d];
+}
+
+void launch_pass_reset(const Params& P, cudaStream_t st) {
+    k_pass_reset<<<(P.max_depth + 256) / 256, 256, 0, st>>>(P);
+}
+
 cudaError_t pass_configure() {
-    return cudaFuncSetAttribute(k_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    return cudaFuncSetAttribute(k_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
 }
 
 int pass_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass, PRE_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PRE_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
     return n;
 }
 
@@ -236,7 +265,10 @@ void launch_tilesum(const Params& P, int grid, cudaStream_t st) {
 }
 
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {
-    if (P.n_tiles) k_pass<<<(uint32_t)grid < P.n_tiles ? grid : P.n_tiles, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
+    if (!P.n_tiles) return;
+    const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
+    if (p == 0) k_pass<true><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else k_pass<false><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
 }
 
 }  // namespace ax
