@@ -45,7 +45,7 @@ struct aceapex_plan_s {
     // device facts
     int device, n_sm, pre_grid, match_ctas_per_sm, fused_grid, pass_grid;
     // scratch layout (byte offsets)
-    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_prog, o_front, o_seg_start, o_seg_cnt, o_dst, o_off, o_len, scratch_bytes;
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_prog, o_front, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
     uint32_t last_launches; int last_strategy;
     int last_cuda;
@@ -162,8 +162,6 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_tiles = o; o += up256(8ull * p->n_tiles);
         p->o_prog = o; o += up256(4ull * p->n_tiles);
         p->o_front = o; o += up256(4ull * (FUSED_MAX_DEPTH + 2));
-        { const size_t nseg = p->max_depth <= FUSED_MAX_DEPTH ? (size_t)p->n_tiles * (FUSED_MAX_DEPTH + 1) : 0;
-          p->o_seg_start = o; o += up256(4ull * nseg); p->o_seg_cnt = o; o += up256(4ull * nseg); }
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
@@ -201,8 +199,6 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
-    P.seg_start = reinterpret_cast<uint32_t*>(s + p->o_seg_start);
-    P.seg_cnt = reinterpret_cast<uint32_t*>(s + p->o_seg_cnt);
     P.prog = reinterpret_cast<uint32_t*>(s + p->o_prog);
     P.front = reinterpret_cast<uint32_t*>(s + p->o_front);
     P.raw_size = p->raw_size; P.block_size = p->block_size; P.n_blocks = p->n_blocks; P.n_tiles = p->n_tiles;

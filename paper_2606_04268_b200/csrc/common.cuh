@@ -21,7 +21,10 @@ constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in share
 
 // ---- match kernel
 constexpr int MATCH_THREADS = 256;                 // k_wave (one launch per depth)
-constexpr int PERSIST_THREADS = 1024;              // k_waves_persistent: one CTA per SM
+#ifndef AX_PT
+#define AX_PT 1024
+#endif
+constexpr int PERSIST_THREADS = AX_PT;             // k_waves: 1024 threads, one CTA per SM (measured best: DESIGN.md 6.2)
 constexpr uint32_t SHORT_MAX = 32;
 constexpr uint32_t FUSED_MAX_DEPTH = 16;           // the fused tile kernel handles streams up to this depth                 // matches up to this length are copied by one thread
 
@@ -57,8 +60,6 @@ struct Params {
     uint32_t* wl_dst;                              // [n_match] match destination (absolute)
     uint32_t* wl_off;                              // [n_match] match source (absolute)
     uint16_t* wl_len;                              // [n_match]
-    uint32_t* seg_start;                           // [n_tiles * (FUSED_MAX_DEPTH+1)] shallow streams: tile's slice start per depth
-    uint32_t* seg_cnt;                             // [n_tiles * (FUSED_MAX_DEPTH+1)] ... and its length
     uint32_t* prog;                                // [n_tiles] fused kernel: phases completed per tile
     uint32_t* front;                               // [FUSED_MAX_DEPTH + 2] fused kernel: leading tiles with prog >= p
     uint64_t raw_size;

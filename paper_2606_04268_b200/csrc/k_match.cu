@@ -56,7 +56,7 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 // source lines are prefetched into L2 and stage k is copied, so after a grid barrier only L2-hit source loads and
 // the stores themselves are on the critical path (DRAM latency on B200 is ~1 us; a wave costs ~3 of them if the
 // entry load, the source load and the barrier are taken one after the other).
-constexpr uint32_t PIECE = 4096;                         // entries per piece (4 per thread)
+constexpr uint32_t PIECE = 4 * PERSIST_THREADS;          // entries per piece (4 per thread)
 constexpr uint32_t NSTAGE = 3;
 constexpr uint32_t OFF_WIN = 1024;                       // wave_off window kept in shared memory
 
@@ -73,7 +73,7 @@ __device__ __forceinline__ void cp_async4(void* smem, const void* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
 
-__global__ void __launch_bounds__(PERSIST_THREADS, 1) k_waves(Params P, uint32_t d_first, uint32_t d_last) {
+__global__ void __launch_bounds__(PERSIST_THREADS, 1024 / PERSIST_THREADS) k_waves(Params P, uint32_t d_first, uint32_t d_last) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WaveSmem& S = *reinterpret_cast<WaveSmem*>(smem_raw);
     if (P.status->fault_flags & F_DEPTH) return;          // wave lists incomplete (k_check_cursors): copy nothing.

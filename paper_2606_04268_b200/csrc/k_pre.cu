@@ -15,7 +15,6 @@ namespace ax {
 struct PreSmem {
     unsigned long long warp_sum[PRE_THREADS / 32];
     uint32_t nloc;                       // entries placed in the tile's sorted list so far
-    uint32_t seg_cnt[FUSED_MAX_DEPTH + 2];   // shallow streams: this tile's matches per depth (-> P.seg_cnt)
     uint32_t e_dst[TILE], e_off[TILE], e_g[TILE];   // the tile's matches grouped by depth; e_g = index in the wave list
     uint16_t e_len[TILE];
     // followed in dynamic shared memory by the depth bins, sized to the stream (pre_bins(max_depth) entries each):
@@ -40,7 +39,6 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
     uint32_t* const s_cnt = reinterpret_cast<uint32_t*>(smem_raw + ((sizeof(PreSmem) + 15) & ~(size_t)15));
     uint32_t* const s_gbase = s_cnt + nbins;
     uint16_t* const s_lbase = reinterpret_cast<uint16_t*>(s_gbase + nbins);
-    const bool shallow = P.max_depth <= FUSED_MAX_DEPTH;     // record per-tile segments for the tiled pass kernel
     if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) s_cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
@@ -49,7 +47,6 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
     for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         __syncthreads();
         if (tid == 0) S.nloc = 0;
-        if (tid <= FUSED_MAX_DEPTH) S.seg_cnt[tid] = 0;
         const uint32_t b = P.prog[tile];
         const unsigned long long tile_prefix = P.tile_state[tile];
         const BlockDesc B = P.blocks[b];
@@ -152,11 +149,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
                     const uint32_t g = atomicAdd(&P.cursor[dp[k]], n);
                     s_gbase[dp[k]] = g;
                     s_lbase[dp[k]] = (uint16_t)atomicAdd(&S.nloc, n);
-                    if (shallow) { S.seg_cnt[dp[k]] = n; P.seg_start[(size_t)tile * (FUSED_MAX_DEPTH + 1) + dp[k]] = g; }
                     s_cnt[dp[k]] = 0;                    // bin is clean again for the next tile
                 }
             __syncthreads();
-            if (shallow && tid >= 1 && tid <= P.max_depth) P.seg_cnt[(size_t)tile * (FUSED_MAX_DEPTH + 1) + tid] = S.seg_cnt[tid];
             // ---- a5: group the tile's entries by depth in shared memory, then write them out in list order so
             // that consecutive threads store consecutive list slots (coalesced runs, one per depth present)
 #pragma unroll
