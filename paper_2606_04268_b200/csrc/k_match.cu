@@ -53,8 +53,8 @@ __device__ __forceinline__ unsigned long long gtime() { unsigned long long t; as
 // ---- the wave kernel: a software pipeline over "pieces" of the wave lists
 // CTA c owns the slice [first + c*per, first + (c+1)*per) of every wave's list, cut into pieces of <= PIECE
 // entries.  Stage k+2's entries travel global -> shared with cp.async (no registers, no stall) while stage k+1's
-// source lines are prefetched into L2 and stage k is copied, so after a grid barrier only L2-hit source loads and
-// the stores themselves are on the critical path (DRAM latency on B200 is ~1 us; a wave costs ~3 of them if the
+// destination lines are prefetched into L2 (the OR-merge is a read-modify-write there) and stage k is copied, so
+// after a grid barrier only the source loads and the merges themselves are on the critical path (DRAM latency on B200 is ~1 us; a wave costs ~3 of them if the
 // entry load, the source load and the barrier are taken one after the other).
 constexpr uint32_t PIECE = 4 * PERSIST_THREADS;          // entries per piece (4 per thread)
 constexpr uint32_t NSTAGE = 3;
@@ -166,18 +166,15 @@ __global__ void __launch_bounds__(PERSIST_THREADS, 1024 / PERSIST_THREADS) k_wav
             asm volatile("cp.async.commit_group;" ::: "memory");   // keep every thread's group count in step
             asm volatile("cp.async.wait_group 1;" ::: "memory");   // (warp 0 took part in the prologue's pieces 0 and 1)
         } else {
-            // warps 1..31, meanwhile: fetch piece k+2, and once piece k+1 has landed pull the next wave's source and
-            // destination lines into L2
+            // warps 1..31, meanwhile: fetch piece k+2, and once piece k+1 has landed pull the next wave's destination
+            // lines into L2 (prefetching the sources too was measured slower: DESIGN.md 6.2)
             issue(pc[s2], s2, tid - 32, NW);
             asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed (this thread's part)
             asm volatile("bar.sync 1, %0;" ::"n"(NW) : "memory");
             if (boundary AX_PREFETCH_COND) {
                 const uint32_t sh = nxt.a & 1u;
                 for (uint32_t i = tid - 32; i < nxt.n; i += NW)
-                    if (S.len[s1][i + sh]) {
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.off[s1][i]));
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.dst[s1][i]));
-                    }
+                    if (S.len[s1][i + sh]) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.dst[s1][i]));
             }
         }
         TRACE(3); TRACE_ARR(2);
