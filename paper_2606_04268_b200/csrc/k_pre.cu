@@ -134,7 +134,18 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
 #pragma unroll
         for (int k = 0; k < PRE_ITEMS; ++k) {
             rank[k] = 0;
-            if (of[k] != 0xFFFFFFFFu) rank[k] = smem_bins ? atomicAdd(&s_cnt[dp[k]], 1u) : atomicAdd(&P.cursor[dp[k]], 1u);
+            if (smem_bins) {
+                if (of[k] != 0xFFFFFFFFu) rank[k] = atomicAdd(&s_cnt[dp[k]], 1u);
+            } else {
+                // streams deeper than the shared-memory bins: one GLOBAL atomic per distinct depth in the warp
+                const bool m = of[k] != 0xFFFFFFFFu;
+                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, m ? dp[k] : 0u);
+                const int leader = __ffs(peers) - 1;
+                uint32_t base = 0;
+                if (m && (int)lane == leader) base = atomicAdd(&P.cursor[dp[k]], (uint32_t)__popc(peers));
+                base = __shfl_sync(0xFFFFFFFFu, base, leader);
+                if (m) rank[k] = base + __popc(peers & ((1u << lane) - 1u));
+            }
         }
         if (smem_bins) {
 #pragma unroll
