@@ -61,8 +61,9 @@ def load_workload(name: str, size_mb: int | None = None, enc_override: dict | No
     try:
         os.makedirs(cache, exist_ok=True)
         for f, a in ((f_raw, raw), (f_comp, comp)):
-            np.save(f + ".tmp.npy", a)
-            os.replace(f + ".tmp.npy", f)
+            tmp = f"{f}.{os.getpid()}.tmp.npy"             # ranks of one job may fill the cache at the same time
+            np.save(tmp, a)
+            os.replace(tmp, f)
     except OSError:
         pass
     return raw, comp

@@ -345,3 +345,30 @@ def test_guard_bands_all_strategies():
             assert bool((big_s[:G] == 0xEE).all()) and bool((big_s[G + sb:] == 0xEE).all()), (kind, strat, "scratch guard")
             assert np.array_equal(big_o[G:G + n].cpu().numpy(), raw), (kind, strat)
             p.close()
+
+
+def test_sparse_depths_empty_waves():
+    """Stored depths may be larger than necessary (any order-preserving labelling decodes correctly): here every
+    depth is doubled, so every odd wave is empty — empty waves, empty passes and histogram entries of 0."""
+    rng = np.random.default_rng(31)
+    for bs, nb in ((4096, 5), (1 << 16, 3)):
+        blocks = random_blocks(rng, bs, nb, max_len=200, max_lit=30, p_match=0.7)
+        deps, _ = py_depths(blocks, bs)
+        exp = py_decode(blocks)
+        # keep the test in the shallow range as well: cut chains deeper than 6 (stored depth 12)
+        pos, nblocks = 0, []
+        for blk, dd in zip(blocks, deps):
+            nb_ = []
+            for (lit, mlen, off), d in zip(blk, dd):
+                pos += len(lit)
+                nb_.append((lit + exp[pos:pos + mlen], 0, 0) if (mlen and d > 6) else (lit, mlen, off))
+                pos += mlen
+            nblocks.append(nb_)
+        deps2, _ = py_depths(nblocks, bs)
+        doubled = [[2 * d for d in dd] for dd in deps2]
+        s = build_stream(nblocks, bs, deps=doubled, min_match=1)
+        assert fused_ok(s)
+        for strat in [0] + ALL_STRATS:
+            got, st = gpu_decode(s, strat)
+            assert got.tobytes() == exp, (bs, strat)
+            assert st["max_depth"] % 2 == 0
