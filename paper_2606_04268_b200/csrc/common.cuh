@@ -20,7 +20,6 @@ constexpr int TILE = PRE_THREADS * PRE_ITEMS;      // 2048
 constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in shared memory; deeper streams use global atomics
 
 // ---- match kernel
-constexpr int MATCH_THREADS = 256;                 // k_wave (one launch per depth)
 #ifndef AX_PT
 #define AX_PT 1024
 #endif
@@ -40,7 +39,7 @@ struct Status {
     uint32_t fault_flags;
     uint32_t fault_block;                          // atomicMin; 0xFFFFFFFF = none
     unsigned long long match_src_bytes;            // M_src counted during PRE
-    uint32_t ticket;                               // dynamic tile counter of k_pre
+    uint32_t ticket;                               // dynamic tile counter of k_fused
     uint32_t n_match_seen;
     uint32_t pad0[26];
     uint32_t barrier;                              // grid barrier counter of the persistent wave kernel
@@ -56,11 +55,12 @@ struct Params {
     uint32_t* wave_off;                            // [max_depth + 2]; wave d list = [wave_off[d], wave_off[d+1])
     uint32_t* cursor;                              // [max_depth + 2]; bucket cursors
     BlockDesc* blocks;                             // [n_blocks]
-    unsigned long long* tile_state;                // [n_tiles] decoupled look-back words
+    unsigned long long* tile_state;                // [n_tiles] k_tilesum: exclusive (out << 32 | lit) prefix of the tile in its block
+                                                   //           (k_fused: its decoupled look-back words)
     uint32_t* wl_dst;                              // [n_match] match destination (absolute)
     uint32_t* wl_off;                              // [n_match] match source (absolute)
     uint16_t* wl_len;                              // [n_match]
-    uint32_t* prog;                                // [n_tiles] fused kernel: phases completed per tile
+    uint32_t* prog;                                // [n_tiles] k_tilesum: block index of the tile (k_fused: phases completed per tile)
     uint32_t* front;                               // [FUSED_MAX_DEPTH + 2] fused kernel: leading tiles with prog >= p
     uint64_t raw_size;
     uint32_t block_size, n_blocks, n_tiles, max_depth, min_match, n_match;

@@ -2,7 +2,8 @@
 // four separate arrays"; docs/FORMAT.md directory).  Reads header + directory + depth histogram from the
 // device-resident compressed buffer and writes, into scratch: one BlockDesc per block (stream addresses,
 // n_seq, n_lit, raw_len, first tile), the per-depth wave list offsets (exclusive prefix of the histogram's
-// match counts) and the bucket cursors; clears the status words and the look-back state of k_pre.
+// match counts) and the bucket cursors; clears the status words, the per-tile words (k_tilesum's prefixes /
+// the fused kernel's look-back state) and the fused kernel's progress flags.
 #include "common.cuh"
 
 namespace ax {
@@ -39,7 +40,7 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* s_warp
 
 __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
     __shared__ uint32_t s_warp[33];
-    if (blockIdx.x != 0) {   // the other CTAs clear the decoupled look-back words of k_pre
+    if (blockIdx.x != 0) {   // the other CTAs clear the per-tile words (fused kernel: look-back state and progress flags)
         const uint32_t n = P.n_tiles, stride = (gridDim.x - 1) * IDX_THREADS;
         for (uint32_t i = (blockIdx.x - 1) * IDX_THREADS + threadIdx.x; i < n; i += stride) { P.tile_state[i] = 0ull; P.prog[i] = 0u; }
         return;

@@ -8,7 +8,7 @@
 //               one launch each (a7: a kernel boundary orders wave p-1 before wave p); a match whose
 //               dep is 0 or above max_depth is copied by no pass and shows up as a histogram mismatch (F_DEPTH).
 // Why: with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
-// and a bucketing kernel (k_pre) whose per-tile chain of ticket -> look-back -> bin reservation runs at ~1 TB/s —
+// and a bucketing kernel (k_pre) that ranks, reserves and scatters every match at ~1 TB/s —
 // whereas re-reading the 10 B/sequence stream is a pure streaming read with no inter-CTA dependency: tiles are
 // assigned statically, prefixes come from k_tilesum, nothing is reserved with atomics.
 // Matches are copied exactly as in the wave kernel (copy.cuh: register funnel shift, OR-merge into the zeroed output).
