@@ -180,12 +180,16 @@ def aggregate_gbs(raw_bytes: int, ms_per_step: float, world: int) -> float:
 
 def ncu_traffic(workload: str):
     """DRAM bytes (read + write) of the match kernel(s) of one step — one k_waves launch, or the k_pass launches of
-    depths 1..D — from the committed ncu capture (profiles/traffic.json), else None."""
+    depths 1..D — from the committed ncu capture summary (profiles/traffic.csv), else None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload, {}).get("match_dram_bytes")
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    return int(row["match_dram_bytes"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def measured_peak() -> tuple[float, str]:
