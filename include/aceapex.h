@@ -48,17 +48,15 @@ enum {
     ACEAPEX_PHASE_ALL = 3
 };
 
-/* wave sequencing strategies (step a7); AUTO picks from the plan's per-depth counts */
+/* wave sequencing strategies (step a7); AUTO picks from the plan's per-depth histogram */
 enum {
     ACEAPEX_WAVES_AUTO = 0,
-    ACEAPEX_WAVES_LAUNCH = 1,     /* one kernel launch per depth on the caller's stream                */
-    ACEAPEX_WAVES_GRAPH = 2,      /* the same launches replayed from a cached CUDA graph */
-    ACEAPEX_WAVES_PERSISTENT = 3, /* one cooperative kernel, grid barrier between depths               */
-    ACEAPEX_WAVES_PASSES = 5,     /* shallow streams (max_depth <= 16): no wave lists; the token stream is re-parsed
-                                     by one streaming kernel per depth (k_pass), prefixes from k_tilesum         */
-    ACEAPEX_WAVES_FUSED = 4       /* shallow streams (max_depth <= 16), phases == ALL only: one kernel does
-                                     parse + scan + literals + all waves per tile, output assembled in shared
-                                     memory, tiles ordered by progress flags; PRE / MATCH alone use the lists */
+    ACEAPEX_WAVES_LAUNCH = 1,     /* wave lists; one kernel launch per depth on the caller's stream          */
+    ACEAPEX_WAVES_GRAPH = 2,      /* the same launches replayed from a cached CUDA graph       */
+    ACEAPEX_WAVES_PERSISTENT = 3, /* wave lists; one cooperative kernel, grid barrier between depths         */
+    ACEAPEX_WAVES_SPAN = 4        /* shallow streams whose last depth holds most matches (depth-limited encoder,
+                                     PAPER.md:228): depths 1 .. D-1 through wave lists, depth D by one streaming
+                                     pass over the token stream that writes the whole output once (k_span)   */
 };
 
 /* device-side token fault bits (aceapex_stats.fault_flags) */
@@ -66,7 +64,9 @@ enum {
     ACEAPEX_F_BLOCK_SUM = 1, /* sum(cmd+len) != raw_len[b] or sum(cmd) != n_lit[b]  (I1)               */
     ACEAPEX_F_SOURCE = 2,    /* off >= mdst, or len < min_match                     (I2)               */
     ACEAPEX_F_DEPTH = 4,     /* dep == 0 on a match, dep > max_depth, or counts != depth histogram     */
-    ACEAPEX_F_PLACEHOLDER = 8/* len == 0 with off != 0 or dep != 0                                     */
+    ACEAPEX_F_PLACEHOLDER = 8,/* len == 0 with off != 0 or dep != 0                                    */
+    ACEAPEX_F_INDEX = 16     /* directory / histogram in comp_dev disagree with what aceapex_plan validated
+                                on the host copy (a different or modified buffer): nothing was decoded   */
 };
 
 typedef struct {

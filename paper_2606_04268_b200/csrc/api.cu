@@ -9,24 +9,18 @@
 #include <vector>
 
 namespace ax {
-void launch_index(const Params& P, int n_sm, cudaStream_t st);
+void launch_index(const Params& P, cudaStream_t st);
+void launch_tilesum(const Params& P, int grid, cudaStream_t st);
 void launch_pre(const Params& P, int grid, cudaStream_t st);
 cudaError_t pre_configure();
-size_t pre_smem_bytes(uint32_t max_depth);
 int pre_max_ctas_per_sm(uint32_t max_depth);
 int match_max_ctas_per_sm();
 cudaError_t waves_configure();
-cudaError_t fused_configure();
-int fused_max_ctas_per_sm();
-void launch_fused(const Params& P, int grid, cudaStream_t st);
-void launch_check_cursors(const Params& P, cudaStream_t st);
-cudaError_t pass_configure();
-int pass_max_ctas_per_sm();
-void launch_tilesum(const Params& P, int grid, cudaStream_t st);
-void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st);
-void launch_pass_reset(const Params& P, cudaStream_t st);
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
+cudaError_t span_configure();
+int span_max_ctas_per_sm();
+void launch_span(const Params& P, uint32_t depth_hi, int grid, cudaStream_t st);
 }  // namespace ax
 
 using namespace ax;
@@ -43,11 +37,11 @@ struct aceapex_plan_s {
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
     uint32_t n_tiles;
     // device facts
-    int device, n_sm, pre_grid, match_ctas_per_sm, fused_grid, pass_grid;
+    int device, n_sm, pre_grid, match_ctas_per_sm, span_grid;
     // scratch layout (byte offsets)
-    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_prog, o_front, o_dst, o_off, o_len, scratch_bytes;
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
-    uint32_t last_launches; int last_strategy;
+    uint32_t last_launches; int last_strategy; bool last_had_match;
     int last_cuda;
     cudaStream_t last_stream;
     cudaStream_t capture_stream = nullptr;
@@ -75,20 +69,16 @@ extern "C" const char* aceapex_strerror(int code) {
     }
 }
 
-// Wave strategy from the per-depth counts: few waves -> one launch each;
-// many waves -> persistent kernel with grid barriers (a launch costs more than a barrier).
+// Wave strategy from the header's per-depth histogram and costs measured on B200:
+//  * SPAN: the last depth is copied by one streaming pass over the whole token stream (k_span) instead of through a wave
+//    list.  That pass costs about as much as listing + copying a quarter of the sequences, so it pays when the last
+//    depth holds at least that many matches — the depth-limited encoder's profile (the limit piles the
+//    matches up at depth D).
+//  * otherwise every depth gets a wave list; more than 8 waves run inside one persistent cooperative kernel (a grid
+//    barrier costs ~1.3 us, a launch 4-6 us), fewer as ordinary launches.
 static int choose_strategy(const aceapex_plan_t* p) {
-    const char* e = getenv("ACEAPEX_WAVES");
-    if (e) {
-        if (!strcmp(e, "launch")) return ACEAPEX_WAVES_LAUNCH;
-        if (!strcmp(e, "graph")) return ACEAPEX_WAVES_GRAPH;
-        if (!strcmp(e, "persistent")) return ACEAPEX_WAVES_PERSISTENT;
-        if (!strcmp(e, "fused") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_FUSED;
-        if (!strcmp(e, "passes") && p->max_depth <= FUSED_MAX_DEPTH) return ACEAPEX_WAVES_PASSES;
-    }
-    // measured on B200: up to 8 waves the list-free pass kernels win (192 vs 152 GB/s on
-    // text1g_d4; the fused tile kernel is latency-bound per tile); deeper streams: lists + persistent wave kernel
-    return p->max_depth <= 8 ? ACEAPEX_WAVES_PASSES : ACEAPEX_WAVES_PERSISTENT;
+    if (p->max_depth >= 1 && p->max_depth <= 64 && p->hist_cnt[p->max_depth] * 4 >= p->total_seq) return ACEAPEX_WAVES_SPAN;
+    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -143,14 +133,12 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, device);
         if (ce == cudaSuccess) ce = pre_configure();
         if (ce == cudaSuccess) ce = waves_configure();
-        if (ce == cudaSuccess) ce = fused_configure();
-        if (ce == cudaSuccess) ce = pass_configure();
+        if (ce == cudaSuccess) ce = span_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
         int pre_occ = pre_max_ctas_per_sm(p->max_depth); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
-        { int fo = fused_max_ctas_per_sm(); if (fo < 1) fo = 1; p->fused_grid = p->n_sm * fo; }
-        { int po = pass_max_ctas_per_sm(); if (po < 1) po = 1; p->pass_grid = p->n_sm * po; }
+        { int so = span_max_ctas_per_sm(); if (so < 1) so = 1; p->span_grid = p->n_sm * so; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
         if (cur >= 0 && cur != device) cudaSetDevice(cur);
         // scratch layout
@@ -160,8 +148,7 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_cursor = o; o += up256(4ull * (p->max_depth + 2));
         p->o_blocks = o; o += up256(sizeof(BlockDesc) * (size_t)nb);
         p->o_tiles = o; o += up256(8ull * p->n_tiles);
-        p->o_prog = o; o += up256(4ull * p->n_tiles);
-        p->o_front = o; o += up256(4ull * (FUSED_MAX_DEPTH + 2));
+        p->o_tblk = o; o += up256(4ull * p->n_tiles);
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
@@ -181,13 +168,13 @@ extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p-
 extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
 
 extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
-    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PASSES) return ACEAPEX_E_ARG;
-    if ((s == ACEAPEX_WAVES_FUSED || s == ACEAPEX_WAVES_PASSES) && p->max_depth > FUSED_MAX_DEPTH) return ACEAPEX_E_ARG;
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_SPAN) return ACEAPEX_E_ARG;
+    if (s == ACEAPEX_WAVES_SPAN && p->max_depth == 0) return ACEAPEX_E_ARG;
     p->strategy_forced = s;
     return ACEAPEX_OK;
 }
 
-static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* out_dev, void* scratch_dev) {
+static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* out_dev, void* scratch_dev, int strategy) {
     Params P;
     uint8_t* s = static_cast<uint8_t*>(scratch_dev);
     P.comp = static_cast<const uint8_t*>(comp_dev); P.out = static_cast<uint8_t*>(out_dev);
@@ -196,66 +183,56 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.cursor = reinterpret_cast<uint32_t*>(s + p->o_cursor);
     P.blocks = reinterpret_cast<BlockDesc*>(s + p->o_blocks);
     P.tile_state = reinterpret_cast<unsigned long long*>(s + p->o_tiles);
+    P.tile_blk = reinterpret_cast<uint32_t*>(s + p->o_tblk);
     P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
-    P.prog = reinterpret_cast<uint32_t*>(s + p->o_prog);
-    P.front = reinterpret_cast<uint32_t*>(s + p->o_front);
-    P.raw_size = p->raw_size; P.block_size = p->block_size; P.n_blocks = p->n_blocks; P.n_tiles = p->n_tiles;
-    P.max_depth = p->max_depth; P.min_match = p->min_match; P.n_match = (uint32_t)p->n_match;
+    P.raw_size = p->raw_size; P.comp_bytes = p->comp_bytes; P.block_size = p->block_size; P.n_blocks = p->n_blocks;
+    P.n_tiles = p->n_tiles; P.max_depth = p->max_depth; P.min_match = p->min_match;
+    // strategy SPAN: the last depth has no wave list (k_span copies it straight from the stream)
+    P.list_hi = strategy == ACEAPEX_WAVES_SPAN ? p->max_depth - 1 : p->max_depth;
+    uint64_t nl = 0;
+    for (uint32_t d = 1; d <= P.list_hi; ++d) nl += p->hist_cnt[d];
+    P.n_list = (uint32_t)nl;
     return P;
 }
 
 // Enqueue the kernels of one decode on `st`; returns the number of kernel launches through *n_launch.
 static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, int strategy, cudaStream_t st, uint32_t* n_launch) {
     uint32_t n = 0;
-    if (p->n_blocks == 0) { *n_launch = 0; return cudaSuccess; }
-    if (strategy == ACEAPEX_WAVES_FUSED && phases == ACEAPEX_PHASE_ALL) {
-        launch_index(P, p->n_sm, st);
-        launch_fused(P, p->fused_grid, st);
-        launch_check_cursors(P, st);
-        *n_launch = 1 + (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
-        return cudaGetLastError();
-    }
-    if (strategy == ACEAPEX_WAVES_PASSES) {
-        // shallow streams without wave lists: the stream is re-parsed by every pass (k_pass.cu)
-        if (phases & ACEAPEX_PHASE_PRE) {
-            cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);   // matches are OR-merged into zeros
-            if (ez != cudaSuccess) return ez;
-            launch_index(P, p->n_sm, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
-            n += 2 + (p->n_tiles ? 1 : 0);
-        }
-        if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
-            // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
-            launch_pass_reset(P, st); ++n;
-            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); ++n; }
-            launch_check_cursors(P, st); ++n;
-        }
-        *n_launch = n;
-        return cudaGetLastError();
-    }
-    if (strategy == ACEAPEX_WAVES_FUSED) strategy = p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;   // PRE / MATCH alone: list path
+    *n_launch = 0;
+    if (p->n_blocks == 0) return cudaSuccess;
+    const bool span = strategy == ACEAPEX_WAVES_SPAN;
     if (phases & ACEAPEX_PHASE_PRE) {
         // the wave kernel OR-merges short matches into the output (copy.cuh merge16): start from zeros
-        cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);
-        if (ez != cudaSuccess) return ez;
-        launch_index(P, p->n_sm, st); ++n;
+        if (P.list_hi) {
+            cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);
+            if (ez != cudaSuccess) return ez;
+        }
+        launch_index(P, st); ++n;
         launch_tilesum(P, p->n_sm * 8, st); ++n;
-        launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (p->max_depth ? 1 : 0);
+        launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (P.list_hi ? 1 : 0);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
-        if (strategy == ACEAPEX_WAVES_PERSISTENT) {
-            cudaError_t e = launch_waves_persistent(P, 1, p->max_depth, p->n_sm * p->match_ctas_per_sm, st);
+        const int wave_grid = p->n_sm * p->match_ctas_per_sm;
+        if (P.list_hi > 8 && strategy != ACEAPEX_WAVES_LAUNCH && strategy != ACEAPEX_WAVES_GRAPH) {
+            cudaError_t e = launch_waves_persistent(P, 1, P.list_hi, wave_grid, st);
             if (e != cudaSuccess) return e;
             ++n;
         } else {
-            for (uint32_t d = 1; d <= p->max_depth; ++d) {
-                cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], p->n_sm * p->match_ctas_per_sm, st);
+            for (uint32_t d = 1; d <= P.list_hi; ++d) {
+                cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], wave_grid, st);
                 if (e != cudaSuccess) return e;
                 if (p->hist_cnt[d]) ++n;
             }
+        }
+        if (span) {
+            // the last depth: one streaming pass writes the whole output (replayable: the count starts from zero)
+            cudaError_t e = cudaMemsetAsync(&P.status->n_final, 0, sizeof(uint32_t), st);
+            if (e != cudaSuccess) return e;
+            launch_span(P, p->max_depth, p->span_grid, st); n += p->n_tiles ? 1 : 0;
         }
     }
     *n_launch = n;
@@ -270,11 +247,18 @@ extern "C" int aceapex_decode(aceapex_plan_t* p, const void* comp_dev, void* out
     if (out_capacity < aceapex_out_bytes(p) || scratch_bytes < p->scratch_bytes) return ACEAPEX_E_CAPACITY;
     if (((uintptr_t)comp_dev | (uintptr_t)out_dev | (uintptr_t)scratch_dev) & 15) return ACEAPEX_E_ALIGN;
     cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    {   // kernel attributes and grid sizes were set up for the plan's device: refuse to launch anywhere else
+        int cur = -1;
+        e = cudaGetDevice(&cur);
+        if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+        if (cur != p->device) return ACEAPEX_E_ARG;
+    }
     p->last_stream = st;
     const int strategy = p->strategy_forced != ACEAPEX_WAVES_AUTO ? p->strategy_forced : p->strategy_auto;
     p->last_strategy = strategy;
-    const Params P = make_params(p, comp_dev, out_dev, scratch_dev);
-    cudaError_t e;
+    p->last_had_match = (phases & ACEAPEX_PHASE_MATCH) != 0;
+    const Params P = make_params(p, comp_dev, out_dev, scratch_dev, strategy);
     if (strategy != ACEAPEX_WAVES_GRAPH) {
         e = enqueue(p, P, phases, strategy, st, &p->last_launches);
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
@@ -347,7 +331,11 @@ extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, ace
         if (e == cudaSuccess) e = cudaMemcpy(&h, static_cast<const uint8_t*>(scratch_dev) + p->o_status, sizeof h, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
         s->match_src_bytes = h.match_src_bytes; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
-        if (h.fault_flags) return ACEAPEX_E_STREAM;
+        // strategy SPAN keeps no list (hence no cursor) for the last depth: its count comes back from the span pass
+        if (!h.fault_flags && p->last_strategy == ACEAPEX_WAVES_SPAN && p->last_had_match && h.n_final != p->hist_cnt[p->max_depth]) {
+            s->fault_flags = F_DEPTH; s->fault_block = 0xFFFFFFFEu;
+        }
+        if (s->fault_flags) return ACEAPEX_E_STREAM;
     }
     return ACEAPEX_OK;
 }

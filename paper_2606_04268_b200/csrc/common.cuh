@@ -11,9 +11,9 @@ constexpr uint32_t HDR_BYTES = 64, DIR_BYTES = 16, HIST_BYTES = 16;
 constexpr uint32_t FLAG_FLATTENED = 1, FLAG_DEPTH_LIMITED = 2, FLAG_HAS_DEP = 4;
 
 // ---- fault bits (include/aceapex.h ACEAPEX_F_*)
-constexpr uint32_t F_BLOCK_SUM = 1, F_SOURCE = 2, F_DEPTH = 4, F_PLACEHOLDER = 8;
+constexpr uint32_t F_BLOCK_SUM = 1, F_SOURCE = 2, F_DEPTH = 4, F_PLACEHOLDER = 8, F_INDEX = 16;
 
-// ---- PRE kernel tiling: one tile = TILE consecutive sequences of one block
+// ---- tiling of the token stream: one tile = TILE consecutive sequences of one block
 constexpr int PRE_THREADS = 256;
 constexpr int PRE_ITEMS = 8;                       // consecutive sequences per thread (8 x u16 = one 16 B load)
 constexpr int TILE = PRE_THREADS * PRE_ITEMS;      // 2048
@@ -24,8 +24,7 @@ constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in share
 #define AX_PT 1024
 #endif
 constexpr int PERSIST_THREADS = AX_PT;             // k_waves: 1024 threads, one CTA per SM (measured best: DESIGN.md 6.2)
-constexpr uint32_t SHORT_MAX = 32;
-constexpr uint32_t FUSED_MAX_DEPTH = 16;           // the fused tile kernel handles streams up to this depth                 // matches up to this length are copied by one thread
+constexpr uint32_t SHORT_MAX = 32;                 // matches up to this length are copied by one thread
 
 // Per-block descriptor written by k_index (step a1).  Stream addresses are byte offsets from comp base.
 struct BlockDesc {
@@ -39,9 +38,8 @@ struct Status {
     uint32_t fault_flags;
     uint32_t fault_block;                          // atomicMin; 0xFFFFFFFF = none
     unsigned long long match_src_bytes;            // M_src counted during PRE
-    uint32_t ticket;                               // dynamic tile counter of k_fused
-    uint32_t n_match_seen;
-    uint32_t pad0[26];
+    uint32_t n_final;                              // matches of the last depth copied by the span pass (histogram check)
+    uint32_t pad0[27];
     uint32_t barrier;                              // grid barrier counter of the persistent wave kernel
     uint32_t pad1[31];
 };
@@ -55,15 +53,16 @@ struct Params {
     uint32_t* wave_off;                            // [max_depth + 2]; wave d list = [wave_off[d], wave_off[d+1])
     uint32_t* cursor;                              // [max_depth + 2]; bucket cursors
     BlockDesc* blocks;                             // [n_blocks]
-    unsigned long long* tile_state;                // [n_tiles] k_tilesum: exclusive (out << 32 | lit) prefix of the tile in its block
-                                                   //           (k_fused: its decoupled look-back words)
-    uint32_t* wl_dst;                              // [n_match] match destination (absolute)
-    uint32_t* wl_off;                              // [n_match] match source (absolute)
-    uint16_t* wl_len;                              // [n_match]
-    uint32_t* prog;                                // [n_tiles] k_tilesum: block index of the tile (k_fused: phases completed per tile)
-    uint32_t* front;                               // [FUSED_MAX_DEPTH + 2] fused kernel: leading tiles with prog >= p
-    uint64_t raw_size;
-    uint32_t block_size, n_blocks, n_tiles, max_depth, min_match, n_match;
+    unsigned long long* tile_state;                // [n_tiles] exclusive (out << 32 | lit) prefix of the tile inside its block
+    uint32_t* tile_blk;                            // [n_tiles] block index of the tile
+    uint32_t* wl_dst;                              // [n_list] match destination (absolute)
+    uint32_t* wl_off;                              // [n_list] match source (absolute)
+    uint16_t* wl_len;                              // [n_list]
+    uint64_t raw_size, comp_bytes;
+    uint32_t block_size, n_blocks, n_tiles, max_depth, min_match;
+    uint32_t n_list;                               // capacity of the wave lists = matches at depths 1 .. list_hi
+    uint32_t list_hi;                              // depths 1 .. list_hi travel through wave lists; deeper ones (strategy
+                                                   // SPAN: the last depth) are copied by the span pass straight from the stream
 };
 
 __host__ __device__ inline uint64_t pad16(uint64_t x) { return (x + 15) & ~(uint64_t)15; }
@@ -71,6 +70,38 @@ __host__ __device__ inline uint64_t pad16(uint64_t x) { return (x + 15) & ~(uint
 __device__ __forceinline__ void raise_fault(Status* st, uint32_t bits, uint32_t block) {
     atomicOr(&st->fault_flags, bits);
     atomicMin(&st->fault_block, block);
+}
+
+// ---- step a2, token parse: the 8 consecutive sequences of one thread from five 16-byte words (cmd, len, dep: 8 x u16;
+// off: 8 x u32 in two words); entries at or past `n_valid` are zeroed (streams are padded to 16 bytes with zeros, but a
+// tile's tail shares its last words with nothing — the mask is what makes them empty).
+struct Seq8 { uint32_t c[PRE_ITEMS], l[PRE_ITEMS], dp[PRE_ITEMS], of[PRE_ITEMS]; };
+
+__device__ __forceinline__ void unpack8(uint4 v, uint32_t (&x)[PRE_ITEMS]) {
+    x[0] = v.x & 0xFFFFu; x[1] = v.x >> 16; x[2] = v.y & 0xFFFFu; x[3] = v.y >> 16;
+    x[4] = v.z & 0xFFFFu; x[5] = v.z >> 16; x[6] = v.w & 0xFFFFu; x[7] = v.w >> 16;
+}
+
+__device__ __forceinline__ void parse8(Seq8& s, uint4 vc, uint4 vl, uint4 vd, uint4 o0, uint4 o1, uint32_t n_valid) {
+    unpack8(vc, s.c); unpack8(vl, s.l); unpack8(vd, s.dp);
+    s.of[0] = o0.x; s.of[1] = o0.y; s.of[2] = o0.z; s.of[3] = o0.w; s.of[4] = o1.x; s.of[5] = o1.y; s.of[6] = o1.z; s.of[7] = o1.w;
+#pragma unroll
+    for (int k = 0; k < PRE_ITEMS; ++k) if ((uint32_t)k >= n_valid) { s.c[k] = 0; s.l[k] = 0; s.dp[k] = 0; s.of[k] = 0; }
+}
+
+// The same from global memory: sequences j0 .. j0+7 of block B (j0 a multiple of 8).  need_src = false skips dep[] / off[].
+__device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const BlockDesc& B, uint32_t j0, bool need_src) {
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+    if (j0 >= B.n_seq) { parse8(s, z, z, z, z, z, 0); return; }
+    const uint4 vc = *reinterpret_cast<const uint4*>(comp + B.cmd_off + 2ull * j0);
+    const uint4 vl = *reinterpret_cast<const uint4*>(comp + B.len_off + 2ull * j0);
+    uint4 vd = z, o0 = z, o1 = z;
+    if (need_src) {
+        vd = *reinterpret_cast<const uint4*>(comp + B.dep_off + 2ull * j0);
+        o0 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0);
+        o1 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0 + 16);
+    }
+    parse8(s, vc, vl, vd, o0, o1, B.n_seq - j0);
 }
 
 // ---- 16-byte funnel shift: bytes [sh, sh+16) of the 32-byte value (a | b << 128), sh in 0..15
@@ -91,29 +122,49 @@ __device__ __forceinline__ uint4 shift16(uint4 a, uint4 b, uint32_t sh) {
     return o;
 }
 
-// ---- warp-cooperative copy of n bytes, source and destination ranges disjoint.
-// dst: 16-byte aligned vector stores on the body, byte stores on head/tail; never stores outside [dst, dst+n).
-// src: whole aligned 16-byte words are loaded (plain L1-cached loads: callers order them after the producing wave
-// by a kernel boundary or an acquiring grid barrier), so up to 15 bytes beyond either end of the source may be READ.
-__device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t lane) {
+// ---- cooperative copy of n bytes by a group of G lanes (gl = lane index inside the group), source and destination
+// ranges disjoint.  dst: 16-byte aligned vector stores on the body, byte stores on head/tail; never stores outside
+// [dst, dst+n).  src: whole aligned 16-byte words are loaded (plain L1-cached loads: callers order them after the
+// producing wave by a kernel boundary or an acquiring grid barrier), so up to 15 bytes beyond either end of the source
+// may be READ.  The body is unrolled by 4 so that four loads per lane are in flight (a long literal run or match is a
+// memcpy: its rate is set by the loads in flight, not by the instruction count).
+template <uint32_t G>
+__device__ __forceinline__ void group_copy(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t gl) {
     uint32_t h = (uint32_t)(-(intptr_t)dst) & 15u;
     if (h > n) h = n;
-    if (lane < h) dst[lane] = src[lane];
+    if (gl < h) dst[gl] = src[gl];
+    if (G < 16 && gl + G < h) dst[gl + G] = src[gl + G];
     dst += h; src += h; n -= h;
     const uint32_t nvec = n >> 4;
     const uint32_t sh = (uint32_t)((uintptr_t)src & 15u);
     const uint4* s16 = reinterpret_cast<const uint4*>(src - sh);
     uint4* d16 = reinterpret_cast<uint4*>(dst);
+    uint32_t v = gl;
     if (sh == 0) {
-        for (uint32_t v = lane; v < nvec; v += 32) d16[v] = s16[v];
+        for (; v + 3 * G < nvec; v += 4 * G) {
+            const uint4 a = s16[v], b = s16[v + G], c = s16[v + 2 * G], d = s16[v + 3 * G];
+            d16[v] = a; d16[v + G] = b; d16[v + 2 * G] = c; d16[v + 3 * G] = d;
+        }
+        for (; v < nvec; v += G) d16[v] = s16[v];
     } else {
-        for (uint32_t v = lane; v < nvec; v += 32) {
+        for (; v + 3 * G < nvec; v += 4 * G) {
+            const uint4 a0 = s16[v], a1 = s16[v + 1], b0 = s16[v + G], b1 = s16[v + G + 1],
+                        c0 = s16[v + 2 * G], c1 = s16[v + 2 * G + 1], e0 = s16[v + 3 * G], e1 = s16[v + 3 * G + 1];
+            d16[v] = shift16(a0, a1, sh); d16[v + G] = shift16(b0, b1, sh);
+            d16[v + 2 * G] = shift16(c0, c1, sh); d16[v + 3 * G] = shift16(e0, e1, sh);
+        }
+        for (; v < nvec; v += G) {
             const uint4 a = s16[v], b = s16[v + 1];
             d16[v] = shift16(a, b, sh);
         }
     }
     const uint32_t t = n & 15u, tb = nvec << 4;
-    if (lane < t) dst[tb + lane] = src[tb + lane];
+    if (gl < t) dst[tb + gl] = src[tb + gl];
+    if (G < 16 && gl + G < t) dst[tb + gl + G] = src[tb + gl + G];
+}
+
+__device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t lane) {
+    group_copy<32>(dst, src, n, lane);
 }
 
 }  // namespace ax

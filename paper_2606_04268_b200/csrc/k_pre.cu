@@ -5,9 +5,10 @@
 //   a4  out[dst[j] .. +cmd[j]) = lit_b[lsrc[j] ..)
 //   a5  matches grouped by dep[j] into per-depth wave lists (mdst, off, len)             (§7.1)
 // One tile = 2048 consecutive sequences of one block.  The block-level part of the scan (the prefix of each tile
-// inside its block) is computed first by k_tilesum (k_pass.cu), so tiles are independent here: static assignment,
-// no ticket, no look-back.  dst[] and lsrc[] are never written to memory.  Used for streams deeper than 8 levels;
-// shallower ones skip the wave lists altogether (k_pass.cu).
+// inside its block) is computed first by k_tilesum, so tiles are independent here: static assignment,
+// no ticket, no look-back.  dst[] and lsrc[] are never written to memory.  Matches of depths 1 .. list_hi get list
+// entries; strategy SPAN (shallow streams) sets list_hi = max_depth - 1 and copies the last depth straight from the
+// stream (k_span.cu).
 #include "common.cuh"
 
 namespace ax {
@@ -39,41 +40,24 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
     uint32_t* const s_cnt = reinterpret_cast<uint32_t*>(smem_raw + ((sizeof(PreSmem) + 15) & ~(size_t)15));
     uint32_t* const s_gbase = s_cnt + nbins;
     uint16_t* const s_lbase = reinterpret_cast<uint16_t*>(s_gbase + nbins);
+    if (P.status->fault_flags & F_INDEX) return;          // the block index is inconsistent (k_index): touch nothing
     if (smem_bins) for (uint32_t i = tid; i <= P.max_depth; i += PRE_THREADS) s_cnt[i] = 0;
     unsigned long long src_bytes = 0;
 
     // Tiles are assigned statically; the per-tile prefix inside the block and the tile -> block map come from
-    // k_tilesum (k_pass.cu), so there is no ticket, no look-back and no dependency between CTAs here.
+    // k_tilesum, so there is no ticket, no look-back and no dependency between CTAs here.
     for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         __syncthreads();
         if (tid == 0) S.nloc = 0;
-        const uint32_t b = P.prog[tile];
+        const uint32_t b = P.tile_blk[tile];
         const unsigned long long tile_prefix = P.tile_state[tile];
         const BlockDesc B = P.blocks[b];
         const uint32_t t_in_blk = tile - B.tile_base;
         const uint32_t j0 = t_in_blk * TILE + tid * PRE_ITEMS;          // first sequence of this thread
         // ---- a2: parse (16-byte loads; streams are padded to 16 bytes, entries past n_seq are masked)
-        uint32_t c[PRE_ITEMS], l[PRE_ITEMS], dp[PRE_ITEMS], of[PRE_ITEMS];
-        if (j0 < B.n_seq) {
-            const uint4 vc = *reinterpret_cast<const uint4*>(P.comp + B.cmd_off + 2ull * j0);
-            const uint4 vl = *reinterpret_cast<const uint4*>(P.comp + B.len_off + 2ull * j0);
-            const uint4 vd = *reinterpret_cast<const uint4*>(P.comp + B.dep_off + 2ull * j0);
-            const uint4 o0 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0);
-            const uint4 o1 = *reinterpret_cast<const uint4*>(P.comp + B.off_off + 4ull * j0 + 16);
-            const uint32_t wc[4] = {vc.x, vc.y, vc.z, vc.w}, wl[4] = {vl.x, vl.y, vl.z, vl.w}, wd[4] = {vd.x, vd.y, vd.z, vd.w};
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                c[2 * k] = wc[k] & 0xFFFFu; c[2 * k + 1] = wc[k] >> 16;
-                l[2 * k] = wl[k] & 0xFFFFu; l[2 * k + 1] = wl[k] >> 16;
-                dp[2 * k] = wd[k] & 0xFFFFu; dp[2 * k + 1] = wd[k] >> 16;
-            }
-            of[0] = o0.x; of[1] = o0.y; of[2] = o0.z; of[3] = o0.w; of[4] = o1.x; of[5] = o1.y; of[6] = o1.z; of[7] = o1.w;
-#pragma unroll
-            for (int k = 0; k < PRE_ITEMS; ++k) if (j0 + k >= B.n_seq) { c[k] = 0; l[k] = 0; dp[k] = 0; of[k] = 0; }
-        } else {
-#pragma unroll
-            for (int k = 0; k < PRE_ITEMS; ++k) { c[k] = 0; l[k] = 0; dp[k] = 0; of[k] = 0; }
-        }
+        Seq8 q;
+        load_seq8(q, P.comp, B, j0, true);
+        uint32_t (&c)[PRE_ITEMS] = q.c, (&l)[PRE_ITEMS] = q.l, (&dp)[PRE_ITEMS] = q.dp, (&of)[PRE_ITEMS] = q.of;
         // ---- a3: scan of (cmd+len, cmd) packed as (hi, lo) of one u64
         unsigned long long tsum = 0;
 #pragma unroll
@@ -125,6 +109,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
                 else if (dp[k] == 0 || dp[k] > P.max_depth) { raise_fault(P.status, F_DEPTH, b); m = false; }
             }
             if (m) { const uint32_t dist = mdst - of[k]; src_bytes += l[k] < dist ? l[k] : dist; }
+            if (dp[k] > P.list_hi) m = false;                // strategy SPAN: the last depth is copied by k_span, no list entry
             of[k] = m ? of[k] : 0xFFFFFFFFu;
             c[k] = mdst;
             pos += l[k];
@@ -199,12 +184,9 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
 // After PRE: every cursor must have reached the end of its list, else the histogram lied (fault F_DEPTH).
 __global__ void k_check_cursors(Params P) {
     const uint32_t d = blockIdx.x * blockDim.x + threadIdx.x + 1;
-    if (d <= P.max_depth && P.cursor[d] != P.wave_off[d + 1]) raise_fault(P.status, F_DEPTH, 0xFFFFFFFEu);
+    if (d <= P.list_hi && P.cursor[d] != P.wave_off[d + 1]) raise_fault(P.status, F_DEPTH, 0xFFFFFFFEu);
 }
 
-void launch_check_cursors(const Params& P, cudaStream_t st) {
-    if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
-}
 
 size_t pre_smem_bytes(uint32_t max_depth) { return pre_smem_for(max_depth); }
 
@@ -220,7 +202,7 @@ int pre_max_ctas_per_sm(uint32_t max_depth) {
 
 void launch_pre(const Params& P, int grid, cudaStream_t st) {
     if (P.n_tiles) k_pre<<<grid, PRE_THREADS, pre_smem_for(P.max_depth), st>>>(P);
-    if (P.max_depth) k_check_cursors<<<(P.max_depth + 255) / 256, 256, 0, st>>>(P);
+    if (P.list_hi) k_check_cursors<<<(P.list_hi + 255) / 256, 256, 0, st>>>(P);
 }
 
 }  // namespace ax

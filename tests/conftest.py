@@ -11,7 +11,6 @@ for p in (ROOT, os.path.dirname(os.path.abspath(__file__))):
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
-    config.addinivalue_line("markers", "full: BASELINE full-size configs (minutes of CPU encode; set ACEAPEX_FULL=1)")
 
 
 @pytest.fixture(scope="session")

@@ -12,13 +12,13 @@ from streams import build_stream, py_decode, py_depths, random_blocks
 
 pytestmark = pytest.mark.gpu
 
-STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]       # the wave-list path, three ways of sequencing
-ALL_STRATS = STRATS + [ax.WAVES_FUSED, ax.WAVES_PASSES]               # + the list-free kernels (max_depth <= 16 only)
+STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]       # wave lists for every depth, three ways of sequencing
+ALL_STRATS = STRATS + [ax.WAVES_SPAN]                                 # + last depth by the streaming span pass (k_span)
 
 
-def fused_ok(comp):
-    """The fused tile kernel accepts streams of max_depth <= 16 (header offset 40)."""
-    return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) <= 16
+def span_ok(comp):
+    """Strategy SPAN needs at least one match depth (header offset 40: max_depth)."""
+    return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) >= 1
 
 
 def gpu_decode(comp, strategy=0, check=True):
@@ -36,7 +36,7 @@ def gpu_decode(comp, strategy=0, check=True):
 def assert_parity(comp, raw=None, strategies=STRATS):
     want = oracle.decode(comp)
     rep = oracle.validate(comp)
-    if strategies is STRATS and fused_ok(comp):
+    if strategies is STRATS and span_ok(comp):
         strategies = ALL_STRATS
     for s in strategies:
         got, st = gpu_decode(comp, s)
@@ -83,7 +83,7 @@ def test_periodic_overlap(k, n):
         blocks = [[(lead + pat, n, len(lead))]]
         s = build_stream(blocks, 1 << 17)
         exp = lead + (pat * (n // k + 2))[:k + n]
-        for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, strat
 
@@ -99,7 +99,7 @@ def test_long_copies_all_alignments():
             seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
     blocks = [seqs]
     s = build_stream(blocks, 1 << 20)
-    for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_LAUNCH):
+    for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
         got, _ = gpu_decode(s, strat)
         assert got.tobytes() == py_decode(blocks), strat
 
@@ -112,7 +112,7 @@ def test_fuzz_streams(bs, nb, seed):
         blocks = random_blocks(rng, bs, nb, max_len=40 if bs < 4096 else 300, max_lit=12 if bs < 4096 else 40)
         s = build_stream(blocks, bs, min_match=1)
         exp = py_decode(blocks)
-        for strat in (ALL_STRATS if fused_ok(s) else STRATS):
+        for strat in (ALL_STRATS if span_ok(s) else STRATS):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, it, strat)
 
@@ -261,38 +261,63 @@ def test_device_faults_are_flagged_not_fatal():
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
 
 
-def _full_size_case(name):
-    """A BASELINE config at full size, in bench.py's launch configuration (AUTO strategy, same buffers): GPU bytes ==
-    generator bytes (which the oracle round trip pins), plus sampled windows against the oracle's decode of the same
-    stream, plus the device-side recount of M_src against the oracle validator's."""
+# ---------------------------------------------------------------- BASELINE configs at full size (bench.py's launch configuration)
+# Every config of BASELINE.json, full size, AUTO strategy, the buffers bench.py uses: the WHOLE output is compared with
+# the oracle's sequential decode (the definition) and with the generator's bytes, and the device-side recount of M_src /
+# n_match with the oracle validator's.  The streams are encoded by the CPU oracle encoder (5-8 MB/s per core): all of
+# them are prepared concurrently, one process each, when the first of these tests runs (about 6 minutes of wall time on
+# the GPU box, then a few seconds per test); bench.py finds them in the same cache afterwards.
+FULL = {   # id -> (workload, encoder overrides)
+    "text256m": ("text256m", {}),
+    "fastq1g": ("fastq1g", {}),
+    "text1g_d4": ("text1g_d4", {}),
+    "stress2g": ("stress2g", {}),                                 # flatten on, D unlimited
+    "stress2g_d4": ("stress2g", {"depth_limit": 4}),              # flatten on, D = 4
+    "stress2g_noflat": ("stress2g", {"flatten": False}),          # flatten OFF: tens of thousands of waves
+}
+
+
+@pytest.fixture(scope="session")
+def full_streams():
+    import subprocess
+    import sys
+    import time
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    t0 = time.time()
+    procs = []
+    for wl, enc in FULL.values():
+        cmd = [sys.executable, os.path.join(root, "bench.py"), "--workload", wl, "--prepare-only"]
+        if "depth_limit" in enc:
+            cmd += ["--depth-limit", str(enc["depth_limit"])]
+        if "flatten" in enc:
+            cmd += ["--flatten", str(int(enc["flatten"]))]
+        procs.append(subprocess.Popen(cmd, cwd=root))
+    for pr in procs:
+        assert pr.wait() == 0
+    print(f"\n[full_streams] {len(procs)} streams generated + encoded concurrently in {time.time() - t0:.0f} s")
+    return True
+
+
+@pytest.mark.parametrize("case", list(FULL))
+def test_full_size(case, full_streams):
     from bench import load_workload
-    raw, comp = load_workload(name)
+    wl, enc = FULL[case]
+    raw, comp = load_workload(wl, None, enc)
     got, st = gpu_decode(comp)
-    assert np.array_equal(got, raw)
-    want = oracle.decode(comp, threads=os.cpu_count() or 1)
-    rng = np.random.default_rng(0)
-    for o in rng.integers(0, raw.size - 4096, 256):
-        assert np.array_equal(got[o:o + 4096], want[o:o + 4096])
+    assert got.size == raw.size
+    want = oracle.decode(comp)                                    # sequential: the definition
+    assert np.array_equal(want, raw)
+    if not np.array_equal(got, want):
+        bad = np.flatnonzero(got != want)
+        raise AssertionError(f"{case}: {bad.size} bytes differ, first at {bad[0]}")
     rep = oracle.validate(comp)
     assert st["match_src_bytes"] == rep["match_src_bytes"] and st["n_match"] == rep["n_match"]
 
 
-def test_full_size_text256m():
-    """BASELINE configs[1] — the workload bench.py times by default (about a minute of CPU encode on a fresh box)."""
-    _full_size_case("text256m")
-
-
-@pytest.mark.full
-@pytest.mark.skipif(not os.environ.get("ACEAPEX_FULL"), reason="1 GiB configs need ~4 min of CPU encode each; set ACEAPEX_FULL=1")
-@pytest.mark.parametrize("name", ["fastq1g", "text1g_d4"])
-def test_full_size_1g(name):
-    _full_size_case(name)
-
-
 @pytest.mark.parametrize("seed", range(4))
-def test_fuzz_shallow_streams_fused(seed):
-    """Encoder-free fuzz restricted to depth <= 16 (sources drawn from literal bytes or shallow matches), so that
-    the fused tile kernel sees random overlaps, tile-straddling sources and multi-tile blocks."""
+def test_fuzz_shallow_streams_span(seed):
+    """Encoder-free fuzz restricted to shallow depths (sources drawn from literal bytes or shallow matches): the
+    span pass sees random overlaps, tile-straddling sources, multi-tile blocks and pieces shorter than a word."""
     rng = np.random.default_rng(900 + seed)
     for bs, nb in ((64, 40), (4096, 6), (1 << 16, 3), (1 << 18, 2)):
         blocks = random_blocks(rng, bs, nb, max_len=60 if bs < 4096 else 400, max_lit=12 if bs < 4096 else 60, p_match=0.7)
@@ -312,8 +337,7 @@ def test_fuzz_shallow_streams_fused(seed):
             nblocks.append(nb_)
         assert py_decode(nblocks) == exp
         s = build_stream(nblocks, bs, min_match=1)
-        assert fused_ok(s)
-        for strat in (ax.WAVES_FUSED, ax.WAVES_PASSES, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, strat)
 
@@ -329,7 +353,7 @@ def test_guard_bands_all_strategies():
     for kind, n, kw in cases:
         raw = workloads.generate(kind, n, 77)
         comp = oracle.encode(raw, **kw)
-        for strat in (ALL_STRATS if fused_ok(comp) else STRATS):
+        for strat in (ALL_STRATS if span_ok(comp) else STRATS):
             p = ax.Plan(comp.ctypes.data, comp.size, 0)
             p.set_strategy(strat)
             cd = torch.from_numpy(comp).cuda()
@@ -367,7 +391,6 @@ def test_sparse_depths_empty_waves():
         deps2, _ = py_depths(nblocks, bs)
         doubled = [[2 * d for d in dd] for dd in deps2]
         s = build_stream(nblocks, bs, deps=doubled, min_match=1)
-        assert fused_ok(s)
         for strat in [0] + ALL_STRATS:
             got, st = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, strat)
