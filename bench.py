@@ -38,7 +38,7 @@ WORKLOADS = {
 }
 TARGETS = ["fastq1g", "text1g_d4"]      # BASELINE.json: "the 1 GB text-like and FASTQ-like workloads"; the first is the headline
 BASE_SEED = 260604268
-STRATEGIES = {"launch": 1, "graph": 2, "persistent": 3, "span": 4}
+STRATEGIES = {"launch": 1, "graph": 2, "persistent": 3, "span": 4, "chain": 5, "passes": 6}
 PAPER_CONTEXT = {"h100_match_phase_gbs": {"enwik9": 44.0, "fastq": 20.3, "enwik9_depth10": 77.2},
                  "source": "PAPER.md:187-188, :206 (one H100 SXM; context, not the target)"}
 
@@ -493,7 +493,7 @@ def main():
     ap.add_argument("--workload", default=None, choices=sorted(WORKLOADS),
                     help="default: both TARGET configs (fastq1g = headline, text1g_d4 under `targets`)")
     ap.add_argument("--size-mb", type=int, default=None, help="development override of the workload size")
-    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent", "span"])
+    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent", "span", "chain", "passes"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--flatten", type=int, default=None, choices=[0, 1], help="encoder override (stress sweep): chain flattening")
     ap.add_argument("--depth-limit", type=int, default=None, help="encoder override (stress sweep): depth limit D, 0 = unlimited")

@@ -54,9 +54,17 @@ enum {
     ACEAPEX_WAVES_LAUNCH = 1,     /* wave lists; one kernel launch per depth on the caller's stream          */
     ACEAPEX_WAVES_GRAPH = 2,      /* the same launches replayed from a cached CUDA graph       */
     ACEAPEX_WAVES_PERSISTENT = 3, /* wave lists; one cooperative kernel, grid barrier between depths         */
-    ACEAPEX_WAVES_SPAN = 4        /* shallow streams whose last depth holds most matches (depth-limited encoder,
+    ACEAPEX_WAVES_SPAN = 4,       /* shallow streams whose last depth holds most matches (depth-limited encoder,
                                      PAPER.md:228): depths 1 .. D-1 through wave lists, depth D by one streaming
                                      pass over the token stream that writes the whole output once (k_span)   */
+    ACEAPEX_WAVES_PASSES = 6,     /* shallow streams (max_depth <= 16, e.g. the depth-limited encoder of PAPER.md:228): no wave
+                                     lists; the token stream is re-parsed once per depth, pass p copying the matches with
+                                     dep == p (k_pass).  E_ARG from aceapex_set_strategy if max_depth > 16          */
+    ACEAPEX_WAVES_CHAIN = 5       /* FLATTENED streams only (after chain flattening no match reads a byte
+                                     another match of its own block produced): no wave lists; ONE pass over the token
+                                     stream in block order copies every match, a tile waiting until all earlier blocks
+                                     are written (k_span<CHAIN>).  E_ARG from aceapex_set_strategy if the header's
+                                     FLATTENED flag is clear                                                    */
 };
 
 /* device-side token fault bits (aceapex_stats.fault_flags) */
@@ -117,7 +125,12 @@ int aceapex_set_strategy(aceapex_plan_t* p, int strategy);
  * All three buffers are owned by the caller and must stay alive until the stream reaches the end of the
  * decode.  One plan must not be in flight on two streams at once.
  * Token-level faults never cause an out-of-bounds access; they are recorded in scratch and surface from
- * aceapex_get_stats as E_STREAM.  Errors here: E_ARG, E_CAPACITY, E_ALIGN, E_CUDA. */
+ * aceapex_get_stats as E_STREAM.  Errors here: E_ARG, E_CAPACITY, E_ALIGN, E_CUDA.
+ * What is NOT checked: dep[] is trusted for scheduling (the device checks only its range and that the per-depth counts
+ * match the header's histogram; under CHAIN also that an in-block source has dep == 1).  A stream whose dep[] understates
+ * a match's true depth — with a histogram to match — lets that match read bytes its wave has not written yet: the output
+ * is then wrong although every access stays in bounds and no fault is raised.  Recomputing depths is the validator's job
+ * (oracle/: invariant I4); a producer that cannot be trusted should be validated before its streams are decoded. */
 int aceapex_decode(aceapex_plan_t* p, const void* comp_dev, void* out_dev, size_t out_capacity,
                    void* scratch_dev, size_t scratch_bytes, unsigned phases, void* stream);
 
@@ -125,7 +138,9 @@ int aceapex_decode(aceapex_plan_t* p, const void* comp_dev, void* out_dev, size_
  * PCIe transfer as the term its timing excludes).  Enqueues on `stream`: H2D copy comp_host -> comp_dev,
  * the full decode, D2H copy out_dev -> out_host (raw_bytes bytes).  comp_host / out_host should be pinned
  * for the copies to be asynchronous; the caller synchronises the stream before reading out_host.
- * comp_dev / out_dev / scratch_dev are caller-owned DEVICE staging buffers, sized and aligned as above. */
+ * comp_dev / out_dev / scratch_dev are caller-owned DEVICE staging buffers, sized and aligned as above.
+ * comp_host must hold the bytes the plan was made from (comp_bytes must equal the planned size; a directory or histogram
+ * that differs from the planned one is caught on the device and reported as ACEAPEX_F_INDEX, nothing being decoded). */
 int aceapex_decode_host(aceapex_plan_t* p, const void* comp_host, size_t comp_bytes, void* out_host,
                         size_t out_host_capacity, void* comp_dev, void* out_dev, size_t out_capacity,
                         void* scratch_dev, size_t scratch_bytes, void* stream);

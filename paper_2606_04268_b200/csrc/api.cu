@@ -12,6 +12,11 @@ namespace ax {
 void launch_index(const Params& P, cudaStream_t st);
 void launch_tilesum(const Params& P, int grid, cudaStream_t st);
 void launch_pre(const Params& P, int grid, cudaStream_t st);
+void launch_check_cursors(const Params& P, cudaStream_t st);
+cudaError_t pass_configure();
+int pass_max_ctas_per_sm();
+void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st);
+void launch_pass_reset(const Params& P, cudaStream_t st);
 cudaError_t pre_configure();
 int pre_max_ctas_per_sm(uint32_t max_depth);
 int match_max_ctas_per_sm();
@@ -21,6 +26,8 @@ cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t 
 cudaError_t span_configure();
 int span_max_ctas_per_sm();
 void launch_span(const Params& P, uint32_t depth_hi, int grid, cudaStream_t st);
+cudaError_t launch_chain(const Params& P, int grid, cudaStream_t st);
+size_t chain_sync_words(uint32_t n_blocks);
 }  // namespace ax
 
 using namespace ax;
@@ -37,9 +44,9 @@ struct aceapex_plan_s {
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
     uint32_t n_tiles;
     // device facts
-    int device, n_sm, pre_grid, match_ctas_per_sm, span_grid;
+    int device, n_sm, pre_grid, match_ctas_per_sm, span_grid, pass_grid;
     // scratch layout (byte offsets)
-    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_dst, o_off, o_len, scratch_bytes;
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_chain, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
     uint32_t last_launches; int last_strategy; bool last_had_match;
     int last_cuda;
@@ -69,16 +76,23 @@ extern "C" const char* aceapex_strerror(int code) {
     }
 }
 
-// Wave strategy from the header's per-depth histogram and costs measured on B200:
-//  * SPAN: the last depth is copied by one streaming pass over the whole token stream (k_span) instead of through a wave
-//    list.  That pass costs about as much as listing + copying a quarter of the sequences, so it pays when the last
-//    depth holds at least that many matches — the depth-limited encoder's profile (the limit piles the
-//    matches up at depth D).
-//  * otherwise every depth gets a wave list; more than 8 waves run inside one persistent cooperative kernel (a grid
-//    barrier costs ~1.3 us, a launch 4-6 us), fewer as ordinary launches.
+// Wave strategy = the cheapest of three cost estimates built from the header (sequences, matches, depths with matches)
+// and per-unit costs measured on B200 (picoseconds per sequence / match, microseconds per wave):
+//   PASSES      literal pass 6.1 ps/seq + per depth one streaming pass 4.0 ps/seq (+ ~3 us launch) + 8.8 ps per match copied
+//   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5 us + 21 ps per match copied from a list
+//   PERSISTENT  the same lists, one cooperative kernel: ~2.8 us of grid barrier + fence drain per depth instead of a launch
+// PASSES is limited to PASS_MAX_DEPTH waves.  SPAN and CHAIN (k_span) are never chosen here: measured slower than the
+// above on every BASELINE config; they stay selectable through aceapex_set_strategy.
 static int choose_strategy(const aceapex_plan_t* p) {
-    if (p->max_depth >= 1 && p->max_depth <= 64 && p->hist_cnt[p->max_depth] * 4 >= p->total_seq) return ACEAPEX_WAVES_SPAN;
-    return p->max_depth <= 8 ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
+    if (p->max_depth == 0) return ACEAPEX_WAVES_LAUNCH;
+    double waves = 0;
+    for (uint32_t d = 1; d <= p->max_depth; ++d) waves += p->hist_cnt[d] != 0;
+    const double seq = (double)p->total_seq, m = (double)p->n_match;
+    const double t_lists = 14.5e-6 * seq + 21e-6 * m;                           // microseconds
+    const double t_launch = t_lists + 5.0 * waves, t_persist = t_lists + 2.8 * waves + 8.0;
+    const double t_passes = p->max_depth <= PASS_MAX_DEPTH ? 6.1e-6 * seq + p->max_depth * (4.0e-6 * seq + 3.0) + 8.8e-6 * m : 1e300;
+    if (t_passes <= t_launch && t_passes <= t_persist) return ACEAPEX_WAVES_PASSES;
+    return t_launch <= t_persist ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -134,11 +148,13 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = pre_configure();
         if (ce == cudaSuccess) ce = waves_configure();
         if (ce == cudaSuccess) ce = span_configure();
+        if (ce == cudaSuccess) ce = pass_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
         int pre_occ = pre_max_ctas_per_sm(p->max_depth); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
         { int so = span_max_ctas_per_sm(); if (so < 1) so = 1; p->span_grid = p->n_sm * so; }
+        { int po = pass_max_ctas_per_sm(); if (po < 1) po = 1; p->pass_grid = p->n_sm * po; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
         if (cur >= 0 && cur != device) cudaSetDevice(cur);
         // scratch layout
@@ -149,6 +165,7 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_blocks = o; o += up256(sizeof(BlockDesc) * (size_t)nb);
         p->o_tiles = o; o += up256(8ull * p->n_tiles);
         p->o_tblk = o; o += up256(4ull * p->n_tiles);
+        p->o_chain = o; o += up256(4ull * chain_sync_words((uint32_t)nb));
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
@@ -168,8 +185,10 @@ extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p-
 extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
 
 extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
-    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_SPAN) return ACEAPEX_E_ARG;
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PASSES) return ACEAPEX_E_ARG;
+    if (s == ACEAPEX_WAVES_PASSES && p->max_depth > PASS_MAX_DEPTH) return ACEAPEX_E_ARG;
     if (s == ACEAPEX_WAVES_SPAN && p->max_depth == 0) return ACEAPEX_E_ARG;
+    if (s == ACEAPEX_WAVES_CHAIN && !(p->flags & FLAG_FLATTENED)) return ACEAPEX_E_ARG;   // needs invariant I3
     p->strategy_forced = s;
     return ACEAPEX_OK;
 }
@@ -184,13 +203,15 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.blocks = reinterpret_cast<BlockDesc*>(s + p->o_blocks);
     P.tile_state = reinterpret_cast<unsigned long long*>(s + p->o_tiles);
     P.tile_blk = reinterpret_cast<uint32_t*>(s + p->o_tblk);
+    P.chain_sync = reinterpret_cast<uint32_t*>(s + p->o_chain);
     P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
     P.raw_size = p->raw_size; P.comp_bytes = p->comp_bytes; P.block_size = p->block_size; P.n_blocks = p->n_blocks;
     P.n_tiles = p->n_tiles; P.max_depth = p->max_depth; P.min_match = p->min_match;
     // strategy SPAN: the last depth has no wave list (k_span copies it straight from the stream)
-    P.list_hi = strategy == ACEAPEX_WAVES_SPAN ? p->max_depth - 1 : p->max_depth;
+    // strategy CHAIN: no wave list at all (k_span<true> copies every match straight from the stream, in block order)
+    P.list_hi = strategy == ACEAPEX_WAVES_CHAIN ? 0 : strategy == ACEAPEX_WAVES_SPAN ? p->max_depth - 1 : p->max_depth;
     uint64_t nl = 0;
     for (uint32_t d = 1; d <= P.list_hi; ++d) nl += p->hist_cnt[d];
     P.n_list = (uint32_t)nl;
@@ -202,7 +223,26 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
     uint32_t n = 0;
     *n_launch = 0;
     if (p->n_blocks == 0) return cudaSuccess;
-    const bool span = strategy == ACEAPEX_WAVES_SPAN;
+    const bool span = strategy == ACEAPEX_WAVES_SPAN, chain = strategy == ACEAPEX_WAVES_CHAIN;
+    if (strategy == ACEAPEX_WAVES_PASSES) {
+        if (phases & ACEAPEX_PHASE_PRE) {
+            // short matches are OR-merged into the output (copy.cuh merge16): start from zeros
+            if (p->max_depth) {
+                cudaError_t ez = cudaMemsetAsync(P.out, 0, (size_t)p->raw_size, st);
+                if (ez != cudaSuccess) return ez;
+            }
+            launch_index(P, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
+            n += 2 + (p->n_tiles ? 1 : 0);
+        }
+        if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
+            // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
+            launch_pass_reset(P, st); ++n;
+            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); n += p->n_tiles ? 1 : 0; }
+            launch_check_cursors(P, st); ++n;
+        }
+        *n_launch = n;
+        return cudaGetLastError();
+    }
     if (phases & ACEAPEX_PHASE_PRE) {
         // the wave kernel OR-merges short matches into the output (copy.cuh merge16): start from zeros
         if (P.list_hi) {
@@ -215,9 +255,15 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
+    if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth && chain) {
+        // one pass over the token stream in block order (replayable: counts and frontier restart from zero)
+        cudaError_t e = cudaMemsetAsync(&P.status->n_final, 0, sizeof(uint32_t), st);
+        if (e == cudaSuccess) e = launch_chain(P, p->span_grid, st);
+        if (e != cudaSuccess) return e;
+        n += p->n_tiles ? 1 : 0;
+    } else if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
         const int wave_grid = p->n_sm * p->match_ctas_per_sm;
-        if (P.list_hi > 8 && strategy != ACEAPEX_WAVES_LAUNCH && strategy != ACEAPEX_WAVES_GRAPH) {
+        if (strategy == ACEAPEX_WAVES_PERSISTENT || (span && P.list_hi > 8)) {
             cudaError_t e = launch_waves_persistent(P, 1, P.list_hi, wave_grid, st);
             if (e != cudaSuccess) return e;
             ++n;
@@ -332,7 +378,9 @@ extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, ace
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
         s->match_src_bytes = h.match_src_bytes; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
         // strategy SPAN keeps no list (hence no cursor) for the last depth: its count comes back from the span pass
-        if (!h.fault_flags && p->last_strategy == ACEAPEX_WAVES_SPAN && p->last_had_match && h.n_final != p->hist_cnt[p->max_depth]) {
+        const uint64_t want_final = p->last_strategy == ACEAPEX_WAVES_SPAN ? p->hist_cnt[p->max_depth] : p->n_match;
+        if (!h.fault_flags && (p->last_strategy == ACEAPEX_WAVES_SPAN || p->last_strategy == ACEAPEX_WAVES_CHAIN) && p->max_depth &&
+            p->last_had_match && h.n_final != want_final) {
             s->fault_flags = F_DEPTH; s->fault_block = 0xFFFFFFFEu;
         }
         if (s->fault_flags) return ACEAPEX_E_STREAM;

@@ -17,6 +17,7 @@ constexpr uint32_t F_BLOCK_SUM = 1, F_SOURCE = 2, F_DEPTH = 4, F_PLACEHOLDER = 8
 constexpr int PRE_THREADS = 256;
 constexpr int PRE_ITEMS = 8;                       // consecutive sequences per thread (8 x u16 = one 16 B load)
 constexpr int TILE = PRE_THREADS * PRE_ITEMS;      // 2048
+constexpr uint32_t PASS_MAX_DEPTH = 16;               // strategy PASSES: one streaming pass per depth, at most this many
 constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in shared memory; deeper streams use global atomics
 
 // ---- match kernel
@@ -55,6 +56,7 @@ struct Params {
     BlockDesc* blocks;                             // [n_blocks]
     unsigned long long* tile_state;                // [n_tiles] exclusive (out << 32 | lit) prefix of the tile inside its block
     uint32_t* tile_blk;                            // [n_tiles] block index of the tile
+    uint32_t* chain_sync;                          // strategy CHAIN: [0] frontier, [32 + b] finished tiles of block b
     uint32_t* wl_dst;                              // [n_list] match destination (absolute)
     uint32_t* wl_off;                              // [n_list] match source (absolute)
     uint16_t* wl_len;                              // [n_list]
@@ -89,8 +91,10 @@ __device__ __forceinline__ void parse8(Seq8& s, uint4 vc, uint4 vl, uint4 vd, ui
     for (int k = 0; k < PRE_ITEMS; ++k) if ((uint32_t)k >= n_valid) { s.c[k] = 0; s.l[k] = 0; s.dp[k] = 0; s.of[k] = 0; }
 }
 
-// The same from global memory: sequences j0 .. j0+7 of block B (j0 a multiple of 8).  need_src = false skips dep[] / off[].
-__device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const BlockDesc& B, uint32_t j0, bool need_src) {
+// The same from global memory: sequences j0 .. j0+7 of block B (j0 a multiple of 8).  need_src = false skips dep[] / off[];
+// sel_depth != 0 loads off[] (32 of the 80 bytes) only if one of the eight sequences sits at that depth — a pass over a
+// sparse depth then reads 6 instead of 10 bytes for most sequences.
+__device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const BlockDesc& B, uint32_t j0, bool need_src, uint32_t sel_depth = 0) {
     const uint4 z = make_uint4(0u, 0u, 0u, 0u);
     if (j0 >= B.n_seq) { parse8(s, z, z, z, z, z, 0); return; }
     const uint4 vc = *reinterpret_cast<const uint4*>(comp + B.cmd_off + 2ull * j0);
@@ -98,8 +102,17 @@ __device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const Bl
     uint4 vd = z, o0 = z, o1 = z;
     if (need_src) {
         vd = *reinterpret_cast<const uint4*>(comp + B.dep_off + 2ull * j0);
-        o0 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0);
-        o1 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0 + 16);
+        bool want = true;
+        if (sel_depth) {
+            const uint32_t lo = sel_depth | (sel_depth << 16);                 // any 16-bit lane of vd equal to sel_depth?
+            const uint32_t x0 = vd.x ^ lo, x1 = vd.y ^ lo, x2 = vd.z ^ lo, x3 = vd.w ^ lo;
+            auto has_zero16 = [](uint32_t x) { return ((x & 0xFFFFu) == 0u) || ((x >> 16) == 0u); };
+            want = has_zero16(x0) || has_zero16(x1) || has_zero16(x2) || has_zero16(x3);
+        }
+        if (want) {
+            o0 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0);
+            o1 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0 + 16);
+        }
     }
     parse8(s, vc, vl, vd, o0, o1, B.n_seq - j0);
 }

@@ -32,23 +32,6 @@ __device__ __forceinline__ void grid_barrier(uint32_t* ctr, uint32_t target) {
     __syncthreads();
 }
 
-#ifdef AX_TRACE
-__device__ unsigned long long ax_trace[8 * 4096];
-__device__ unsigned long long ax_arr[3 * 64 * 160];
-#define TRACE_ARR(which) do { if (tid == 0 && k < 64) ax_arr[((which) * 64 + k) * 160 + cta] = gtime(); } while (0)
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TRACE(slot) do { if (cta == 0 && tid == 0 && k < 4096) ax_trace[8 * k + (slot)] = gtime(); } while (0)
-#else
-#define TRACE(slot) do {} while (0)
-#define TRACE_ARR(which) do {} while (0)
-#endif
-
-#ifdef AX_NO_PREFETCH
-#define AX_PREFETCH_COND && false
-#else
-#define AX_PREFETCH_COND
-#endif
-
 // ---- the wave kernel: a software pipeline over "pieces" of the wave lists
 // CTA c owns the slice [first + c*per, first + (c+1)*per) of every wave's list, cut into pieces of <= PIECE
 // entries.  Stage k+2's entries travel global -> shared with cp.async (no registers, no stall) while stage k+1's
@@ -138,11 +121,8 @@ __global__ void __launch_bounds__(PERSIST_THREADS, 1024 / PERSIST_THREADS) k_wav
     for (uint32_t k = 0; pc[k % NSTAGE].valid; ++k) {
         const uint32_t s0 = k % NSTAGE, s1 = (k + 1) % NSTAGE, s2 = (k + 2) % NSTAGE;
         const Piece cur = pc[s0];
-        TRACE(0); TRACE_ARR(0);
         process(cur, s0);
-        TRACE(1);
         __syncthreads();                                   // every store of this piece is issued; stage s0 is free
-        TRACE(2); TRACE_ARR(1);
         const Piece nxt = pc[s1];
         const bool boundary = nxt.valid && nxt.first_of_wave;   // a7: the next piece opens a new wave
         if (boundary) epoch += nct;
@@ -164,15 +144,13 @@ __global__ void __launch_bounds__(PERSIST_THREADS, 1024 / PERSIST_THREADS) k_wav
             issue(pc[s2], s2, tid - 32, NW);
             asm volatile("cp.async.wait_group 1;" ::: "memory");   // piece k+1 landed (this thread's part)
             asm volatile("bar.sync 1, %0;" ::"n"(NW) : "memory");
-            if (boundary AX_PREFETCH_COND) {
+            if (boundary && k != 0) {                      // (k == 0: piece 1 was issued by all 32 warps, warp 0's part may not have landed)
                 const uint32_t sh = nxt.a & 1u;
                 for (uint32_t i = tid - 32; i < nxt.n; i += NW)
                     if (S.len[s1][i + sh]) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.out + S.dst[s1][i]));
             }
         }
-        TRACE(3); TRACE_ARR(2);
         __syncthreads();
-        TRACE(4);
     }
 }
 
@@ -207,12 +185,3 @@ cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t 
 }
 
 }  // namespace ax
-
-#ifdef AX_TRACE
-extern "C" int aceapex_trace_read(unsigned long long* host, size_t n) {   // debug builds only (-DAX_TRACE)
-    return (int)cudaMemcpyFromSymbol(host, ax::ax_trace, n * sizeof(unsigned long long));
-}
-extern "C" int aceapex_trace_read_arr(unsigned long long* host, size_t n) {
-    return (int)cudaMemcpyFromSymbol(host, ax::ax_arr, n * sizeof(unsigned long long));
-}
-#endif

@@ -1,0 +1,186 @@
+// k_pass.cu — strategy PASSES for shallow streams (e.g. the depth-limited encoder of PAPER.md:228 §7.4, "at most D
+// match waves"): no wave lists at all.  The token stream is parsed once per pass instead:
+//   k_pass 0    parse cmd[], len[] (a2) + scan inside the tile (a3) + literal scatter (a4).
+//   k_pass p    parse + scan + validation (I2), M_src and copy of the matches with dep == p (a6), p = 1 .. max_depth,
+//               one launch each (a7: a kernel boundary orders wave p-1 before wave p); a match whose
+//               dep is 0 or above max_depth is copied by no pass and shows up as a histogram mismatch (F_DEPTH).
+// Why: with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
+// and a bucketing kernel (k_pre) that ranks, reserves and scatters every match — whereas re-reading the 10 B/sequence
+// stream is a pure streaming read with no inter-CTA dependency: tiles are assigned statically, their prefixes inside the
+// block come from k_tilesum, nothing is reserved with atomics.
+// Matches are copied exactly as in the wave kernel (copy.cuh: register funnel shift, OR-merge into the zeroed output).
+#include "common.cuh"
+#include "copy.cuh"
+
+namespace ax {
+
+constexpr int PS_WARPS = PRE_THREADS / 32;
+constexpr int PS_WCAP = 32 * PRE_ITEMS;                  // matches one warp can select in a tile (256)
+
+struct PassSmem {
+    unsigned long long warp_sum[PS_WARPS];
+    uint32_t cnt;                                        // matches this CTA copied in this pass (histogram check)
+    uint32_t w_dst[PS_WARPS][PS_WCAP];                   // per warp: the tile's matches of this pass, compacted
+    uint32_t w_off[PS_WARPS][PS_WCAP];
+    uint16_t w_len[PS_WARPS][PS_WCAP];
+};
+
+// ---- pass p: 0 = literals, p >= 1 = matches of depth p
+template <bool LIT>
+__global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pass(Params P, uint32_t p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PassSmem& S = *reinterpret_cast<PassSmem*>(smem_raw);
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    unsigned long long src_bytes = 0;
+    if (P.status->fault_flags & F_INDEX) return;                    // the block index is inconsistent (k_index): touch nothing
+    if (!LIT && P.status->fault_flags != 0) return;                 // a faulty stream is flagged, not decoded further
+    if (tid == 0) S.cnt = 0;
+    __syncthreads();
+    for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
+        const uint32_t b = P.tile_blk[tile];
+        const unsigned long long pre = P.tile_state[tile];
+        const BlockDesc B = P.blocks[b];
+        const uint32_t j0 = (tile - B.tile_base) * TILE + tid * PRE_ITEMS;
+        // ---- a2: parse (pass 0 needs neither depths nor sources)
+        Seq8 q;
+        load_seq8(q, P.comp, B, j0, !LIT, p == P.max_depth ? 0u : p);     // (the last pass checks every placeholder: it needs every off[])
+        uint32_t (&c)[PRE_ITEMS] = q.c, (&l)[PRE_ITEMS] = q.l, (&dp)[PRE_ITEMS] = q.dp, (&of)[PRE_ITEMS] = q.of;
+        // ---- a3: scan inside the tile; the block-level prefix comes from k_tilesum.  The literal pass scans the pair
+        // (cmd+len, cmd) packed in one u64; match passes need output positions only (32-bit shuffles)
+        uint32_t pos, lsrc = 0;
+        if (LIT) {
+            unsigned long long tsum = 0;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) tsum += ((unsigned long long)(c[k] + l[k]) << 32) | c[k];
+            unsigned long long inc = tsum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            __syncthreads();                             // previous tile's readers of warp_sum are done
+            if (lane == 31) S.warp_sum[warp] = inc;
+            __syncthreads();
+            unsigned long long wpre = 0;
+#pragma unroll
+            for (int w = 0; w < PS_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
+            const unsigned long long ex = pre + wpre + (inc - tsum);
+            pos = (uint32_t)(ex >> 32);                  // output offset inside the block
+            lsrc = (uint32_t)ex;                         // offset inside the block's lit[]
+        } else {
+            uint32_t tsum = 0;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) tsum += c[k] + l[k];
+            uint32_t inc = tsum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                if (lane >= d) inc += t;
+            }
+            __syncthreads();
+            if (lane == 31) S.warp_sum[warp] = inc;
+            __syncthreads();
+            uint32_t wpre = 0;
+#pragma unroll
+            for (int w = 0; w < PS_WARPS; ++w) if (w < (int)warp) wpre += (uint32_t)S.warp_sum[w];
+            pos = (uint32_t)(pre >> 32) + wpre + (inc - tsum);
+        }
+        const uint32_t blk_lo = (uint32_t)B.out_base;
+        if (LIT) {
+            // ---- a4 literal scatter (token validation, M_src and the per-depth counts are taken by the pass that
+            // copies the match: pass 0 reads only cmd[], len[] and lit[]).  Runs of up to 16 bytes: one thread, byte by
+            // byte (the typical run on compressible data is 1-2 bytes); longer runs: the whole warp, 16-byte vector stores.
+            const uint8_t* lit = P.comp + B.lit_off;
+            uint8_t* outb = P.out + B.out_base;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) {
+                const bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len && (uint64_t)lsrc + c[k] <= B.n_lit;
+                if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
+                const uint32_t cc = ok ? c[k] : 0;
+                if (__any_sync(0xFFFFFFFFu, cc != 0)) {  // literal runs are rare on compressible data: skip as a warp
+                    if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
+                    uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
+                    while (longm) {
+                        const int sl = __ffs(longm) - 1; longm &= longm - 1;
+                        const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, sl), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, sl),
+                                       n2 = __shfl_sync(0xFFFFFFFFu, cc, sl);
+                        warp_copy(outb + p2, lit + s2, n2, lane);
+                    }
+                }
+                pos += c[k] + l[k]; lsrc += c[k];
+            }
+        } else {
+            // ---- a6: select this pass's matches (same validity rule as pass 0), compact them per warp, copy
+            uint32_t at = 0, sb = 0;
+#pragma unroll
+            for (int k = 0; k < PRE_ITEMS; ++k) {
+                const bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len;
+                pos += c[k];
+                const uint32_t mdst = blk_lo + pos;
+                bool sel = ok && l[k] != 0 && dp[k] == p;
+                if (sel && (of[k] >= mdst || l[k] < P.min_match)) { raise_fault(P.status, F_SOURCE, b); sel = false; }   // I2
+                if (p == P.max_depth && l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
+                if (sel) { const uint32_t dist = mdst - of[k]; sb += l[k] < dist ? l[k] : dist; }
+                const uint32_t msk = __ballot_sync(0xFFFFFFFFu, sel);
+                if (sel) {
+                    const uint32_t i = at + __popc(msk & ((1u << lane) - 1u));
+                    S.w_dst[warp][i] = mdst; S.w_off[warp][i] = of[k]; S.w_len[warp][i] = (uint16_t)l[k];
+                }
+                at += __popc(msk);
+                pos += l[k];
+            }
+            src_bytes += sb;
+            if (lane == 0 && at) atomicAdd(&S.cnt, at);
+            __syncwarp();
+            // one entry per lane and step (measured on text1g_d4: 3.99 / 4.16 / 4.74 ms for 1 / 2 / 4 entries per lane)
+            for (uint32_t base = 0; base < at; base += 32) {
+                Ent e[1];
+                const uint32_t i = base + lane;
+                e[0].mdst = 0; e[0].off = 0; e[0].len = 0;
+                if (i < at) { e[0].mdst = S.w_dst[warp][i]; e[0].off = S.w_off[warp][i]; e[0].len = S.w_len[warp][i]; }
+                copy_ents<1>(P.out, e, lane);
+            }
+            __syncwarp();
+        }
+    }
+    if (!LIT) {
+        __syncthreads();
+        if (tid == 0 && S.cnt) atomicAdd(&P.cursor[p], S.cnt);      // histogram check (k_check_cursors after the last pass)
+#pragma unroll
+        for (int d = 16; d; d >>= 1) src_bytes += __shfl_xor_sync(0xFFFFFFFFu, src_bytes, d);
+        if (lane == 0 && src_bytes) atomicAdd(&P.status->match_src_bytes, src_bytes);
+    }
+}
+
+// Before the match passes of a step: the counters they accumulate start from the header's offsets again, so that
+// PHASE_MATCH can be replayed on its own (this is how the match phase is timed alone).
+__global__ void k_pass_reset(Params P) {
+    const uint32_t d = blockIdx.x * blockDim.x + threadIdx.x;
+    if (d == 0) P.status->match_src_bytes = 0ull;
+    if (d >= 1 && d <= P.max_depth) P.cursor[d] = P.wave_off[d];
+}
+
+void launch_pass_reset(const Params& P, cudaStream_t st) {
+    k_pass_reset<<<(P.max_depth + 256) / 256, 256, 0, st>>>(P);
+}
+
+cudaError_t pass_configure() {
+    cudaError_t e = cudaFuncSetAttribute(k_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+}
+
+int pass_max_ctas_per_sm() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PRE_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
+    return n;
+}
+
+void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {
+    if (!P.n_tiles) return;
+    const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
+    if (p == 0) k_pass<true><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else k_pass<false><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
+}
+
+}  // namespace ax

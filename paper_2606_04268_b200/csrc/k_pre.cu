@@ -10,6 +10,7 @@
 // entries; strategy SPAN (shallow streams) sets list_hi = max_depth - 1 and copies the last depth straight from the
 // stream (k_span.cu).
 #include "common.cuh"
+#include "copy.cuh"
 
 namespace ax {
 
@@ -31,7 +32,7 @@ __host__ __device__ inline size_t pre_smem_for(uint32_t max_depth) {
     return ((sizeof(PreSmem) + 15) & ~(size_t)15) + (size_t)pre_bins(max_depth) * 10u;
 }
 
-__global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
+__global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pre(Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PreSmem& S = *reinterpret_cast<PreSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -91,7 +92,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 4) k_pre(Params P) {
             if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
             const uint32_t cc = ok ? c[k] : 0;
             if (__any_sync(0xFFFFFFFFu, cc != 0)) {          // literal runs are rare on compressible data: skip as a warp
-                if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }
+                if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
                 uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
                 while (longm) {                              // long runs by the whole warp
                     const int src_lane = __ffs(longm) - 1; longm &= longm - 1;
@@ -200,9 +201,13 @@ int pre_max_ctas_per_sm(uint32_t max_depth) {
     return n;
 }
 
+void launch_check_cursors(const Params& P, cudaStream_t st) {
+    if (P.list_hi) k_check_cursors<<<(P.list_hi + 255) / 256, 256, 0, st>>>(P);
+}
+
 void launch_pre(const Params& P, int grid, cudaStream_t st) {
     if (P.n_tiles) k_pre<<<grid, PRE_THREADS, pre_smem_for(P.max_depth), st>>>(P);
-    if (P.list_hi) k_check_cursors<<<(P.list_hi + 255) / 256, 256, 0, st>>>(P);
+    launch_check_cursors(P, st);
 }
 
 }  // namespace ax

@@ -1,50 +1,87 @@
-// k_span.cu — strategy SPAN, the last match wave of a shallow stream (e.g. the depth-limited encoder of PAPER.md:228
-// §7.4, where the depth limit piles most matches up at depth D) as ONE streaming pass over the token stream that
-// writes every output byte exactly once, coalesced, with no wave list, no atomics and no zeroed output:
-//   a2  parse: the tile's cmd[] / len[] / dep[] / off[] slices arrive in shared memory by 1-D bulk TMA
-//       (cp.async.bulk + mbarrier), double-buffered: the next tile's 20 KB are in flight while this one is copied
-//   a3  scan inside the tile (warp shuffles); the tile's prefix inside its block comes from k_tilesum
-//   a6  every token of the tile is materialised into a shared-memory IMAGE of the tile's output span:
-//         literal run              <- lit[]
-//         match with dep == D      <- out[off ..)   (its sources were written by the earlier waves)
-//         match with dep <  D      <- out[mdst ..)  (its own bytes, already written by its wave)
-//       then the image goes to global memory with one bulk TMA store (16-byte chunks; <= 15 head / tail bytes by
-//       byte stores).  Each thread owns 8 consecutive sequences, i.e. one contiguous piece of the span, and assembles it
-//       with a register byte-stream writer: whole 8-byte words go to the image with plain shared-memory stores, the
-//       partial word at each thread boundary travels to its neighbour by shuffle (no shared-memory atomics).
-// Threads whose piece would end beyond the image capacity (tiles with long matches / runs) write their depth-D matches
-// straight to global memory instead (everything else of theirs is there already).
-// Rewriting a byte of depth < D with its own value while another CTA reads it as a match source is harmless: a
-// reader sees the old or the new copy of the same value.
+// k_span.cu — the tile pass: one streaming pass over the token stream that writes every output byte of its matches
+// exactly once, coalesced, with no wave list, no atomics on the output and no zeroed output.  Two uses:
+//   strategy SPAN  (CHAIN = false)  the LAST match wave of a shallow stream (the depth-limited encoder of PAPER.md:228 §7.4
+//       piles most matches up at depth D): depths 1 .. D-1 went through wave lists, this pass copies depth D.
+//   strategy CHAIN (CHAIN = true)   EVERY match of a FLATTENED stream: after chain flattening no match reads bytes
+//       produced by another match of its own block (§3.3, invariant I3), so once the literal scatter has
+//       run, every match of block b depends on blocks < b only.  Tiles are taken in file order; a tile that holds a
+//       match of depth > 1 with a source before its block waits for the FRONTIER (number of leading blocks completely
+//       written) to reach its block; the tile that completes block b publishes frontier = b + 1.  One flag hop per 1 MB
+//       block replaces one grid barrier per depth ("synchronization-bound"); dep[] is used only to skip
+//       the wait (dep == 1: all sources are literals).
+// Per tile (2048 sequences of one block, 512 threads, 2 CTAs per SM):
+//   a2  the tile's cmd[] / len[] / dep[] / off[] slices and its slice of lit[] arrive in shared memory by 1-D bulk TMA
+//       (cp.async.bulk + mbarrier); the next tile's descriptor is fetched by one thread while this tile is processed
+//   a3  scan inside the tile: each thread sums 4 CONSECUTIVE sequences, warp shuffles + one barrier give every token's
+//       output position and literal offset (the tile's prefix inside its block comes from k_tilesum), kept in shared memory
+//   a6  then thread t takes tokens t, t+512, ... (neighbouring lanes = neighbouring tokens: neighbouring sources share
+//       L1 lines, neighbouring destinations share image words):
+//         gather   the aligned 8-byte words holding each short match's source travel global -> shared with cp.async
+//                  (no registers held across the round trip; all of a thread's tokens in flight at once)
+//         assemble every token is written into a shared-memory IMAGE of the tile's output span with naturally aligned
+//                  1/2/4/8-byte stores (each byte has one owner: no merge, no zero fill):
+//                    literal run          <- lit[]
+//                    match being copied   <- out[off ..), periodic if it overlaps   (Q3)
+//                    other matches (SPAN) <- out[mdst ..) (their own bytes, already written by their wave)
+//                  tokens longer than 16 bytes are copied by the whole warp
+//       and the image goes to global memory with one bulk TMA store (16-byte chunks; <= 15 head / tail bytes by byte
+//       stores).  Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight
+//       to global memory instead.
+// Rewriting a byte with its own value while another CTA reads it as a match source is harmless: a reader sees the old
+// or the new copy of the same value.
 #include "common.cuh"
 #include "copy.cuh"
 
 namespace ax {
 
-constexpr int SP_THREADS = PRE_THREADS;              // 256 threads x 8 sequences = one tile per CTA step
+constexpr int SP_PER = 4;                            // tokens per thread
+constexpr int SP_THREADS = TILE / SP_PER;            // 512
 constexpr int SP_WARPS = SP_THREADS / 32;
+constexpr int SP_OCC = 4096 / TILE;                  // CTAs per SM the shared-memory layout below is sized for (2 at TILE = 2048)
 constexpr uint32_t SP_STRM = TILE * 10u;             // cmd | len | dep (2 B each) | off (4 B) per sequence
 constexpr uint32_t SP_O_LEN = TILE * 2u, SP_O_DEP = TILE * 4u, SP_O_OFF = TILE * 6u;
 #ifndef AX_SP_IMG
-#define AX_SP_IMG (28 * 1024)
+#define AX_SP_IMG (10 * TILE)
 #endif
-constexpr uint32_t SP_IMG = AX_SP_IMG;               // image capacity in bytes (a text / FASTQ tile spans ~12 KB)
-constexpr uint32_t KEY_NONE = 0xFFFFFFFFu;
-#ifndef AX_SP_OCC
-#define AX_SP_OCC 2
-#endif
+constexpr uint32_t SP_IMG = AX_SP_IMG;               // image capacity in bytes (a text / FASTQ tile of 2048 sequences spans ~12 KB)
+constexpr uint32_t SP_LIT = 2 * TILE;                // staged slice of the block's lit[] (a text tile holds ~400 literal bytes)
+constexpr uint32_t SP_SHORT = 16;                    // tokens up to this length are copied by one thread
+static_assert(SP_THREADS % 32 == 0 && SP_THREADS * SP_PER == TILE, "one tile per CTA step, 4 sequences per thread");
+
+// What one tile needs, gathered by the thread that issues its loads (while the previous tile is processed), so that the
+// CTA does not walk tile_blk[] -> blocks[] -> tile_state[] (dependent global loads) on its critical path.
+struct TileMeta {
+    unsigned long long pre;                          // (out << 32 | lit) prefix of the tile inside its block
+    const uint8_t* lit;                              // the block's lit[] in global memory
+    uint32_t b, blk_lo, nt, blk_tiles;               // block, its first output byte, sequences in the tile, tiles in the block
+    uint32_t lit16, lit_ok;                          // slit[0] = lit[lit16]; lit_ok: the tile's literal bytes are staged
+};
+
+// Descriptor of the NEXT tile, fetched by one thread straight into shared memory with cp.async (no registers held while
+// it travels), in two steps so that the dependent loads (block descriptor after block index) are issued early and
+// consumed late.
+struct alignas(16) TileFetch {
+    BlockDesc B;                                     // 64 bytes, 16-byte aligned in scratch
+    unsigned long long pre, pre1;                    // tile_state[tile], tile_state[tile + 1]
+    uint32_t b, pad[3];
+};
+static_assert(sizeof(BlockDesc) == 64, "BlockDesc travels as four 16-byte cp.async");
 
 struct SpanSmem {
-    alignas(128) uint8_t strm[2][SP_STRM];
+    alignas(128) uint8_t strm[SP_STRM];
+    alignas(128) uint8_t slit[SP_LIT + 32];
+    alignas(16) uint32_t pos[TILE];                  // absolute output position of token j's literal run; later its source address
+    alignas(16) uint32_t lpos[TILE];                 // offset of token j's literal run inside the block's lit[]; later its copy info
+    alignas(16) unsigned long long x0[TILE], x1[TILE], x2[TILE];   // the aligned words holding token j's source bytes
     alignas(128) uint8_t img[SP_IMG + 64];
-    alignas(8) unsigned long long mbar[2];
+    alignas(8) unsigned long long mbar;
+    TileFetch fetch;                                 // (thread 0) descriptor of the next tile
+    TileMeta meta;
     unsigned long long warp_sum[SP_WARPS];
-    unsigned long long tail_val[SP_WARPS];           // per warp: lane 31's chained partial word ...
-    uint32_t tail_key[SP_WARPS];                     // ... the image word it belongs to ...
-    uint32_t head_key[SP_WARPS];                     // ... and the first image word of the warp's lane 0
-    uint32_t n_img[SP_WARPS];                        // image-mode threads per warp
-    uint32_t img_end[2];                             // absolute end of the span held by the image (slot = iteration parity)
+    uint32_t img_end;                                // absolute end of the span held by the image
 };
+
+static_assert(sizeof(SpanSmem) + 1024 <= (228 * 1024) / SP_OCC, "SP_OCC CTAs (+1 KB reserved each) must fit the 228 KB of one SM");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -71,116 +108,133 @@ __device__ __forceinline__ void bulk_store(void* gmem, const void* smem, uint32_
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gmem), "r"(smem_u32(smem)), "r"(bytes) : "memory");
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+}
 
-// The tile's four stream slices -> stage `st` (one elected thread).  Slices start on 4096-byte multiples of 16-byte
-// aligned streams and are padded to 16 bytes inside the payload (docs/FORMAT.md), so sizes round up to 16 safely.
-__device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, uint32_t tile, uint32_t st) {
-    const uint32_t b = P.tile_blk[tile];
-    const BlockDesc* B = P.blocks + b;
-    const uint32_t j0 = (tile - B->tile_base) * TILE;
-    const uint32_t left = B->n_seq - j0, n = left < (uint32_t)TILE ? left : (uint32_t)TILE;
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void fetch_step1(const Params& P, TileFetch& F, uint32_t tile) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(&F.b)), "l"(P.tile_blk + tile) : "memory");
+    cp_async8(&F.pre, P.tile_state + tile);
+    if (tile + 1 < P.n_tiles) cp_async8(&F.pre1, P.tile_state + tile + 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void fetch_step2(const Params& P, TileFetch& F) {
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    const uint8_t* src = reinterpret_cast<const uint8_t*>(P.blocks + F.b);
+    uint8_t* dst = reinterpret_cast<uint8_t*>(&F.B);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) cp_async16(dst + 16 * i, src + 16 * i);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
+// The tile's stream slices (and its slice of lit[]) -> the stage, and its TileMeta (one elected thread).  Slices start on
+// 4096-byte multiples of 16-byte aligned streams and are padded to 16 bytes inside the payload (docs/FORMAT.md), so sizes
+// round up to 16 safely.  The arrive (release) orders the meta stores before any waiter's reads (acquire).
+__device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, uint32_t tile, const TileFetch& F) {
+    const uint32_t j0 = (tile - F.B.tile_base) * TILE;
+    const uint32_t left = F.B.n_seq - j0, n = left < (uint32_t)TILE ? left : (uint32_t)TILE;
+    const uint32_t lit_lo = (uint32_t)F.pre, lit_hi = j0 + n < F.B.n_seq ? (uint32_t)F.pre1 : F.B.n_lit;
+    const uint32_t l16 = lit_lo & ~15u;
+    const uint32_t lbytes = lit_hi >= lit_lo ? (uint32_t)pad16(lit_hi) - l16 : 0xFFFFFFFFu;
+    const bool lit_ok = lbytes <= SP_LIT;
+    TileMeta& M = S.meta;
+    M.pre = F.pre; M.lit = P.comp + F.B.lit_off; M.b = F.b; M.blk_lo = (uint32_t)F.B.out_base; M.nt = n;
+    M.blk_tiles = (F.B.n_seq + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
     const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
-    mbar_expect_tx(&S.mbar[st], 3 * b2 + b4);
-    bulk_load(S.strm[st], P.comp + B->cmd_off + 2ull * j0, b2, &S.mbar[st]);
-    bulk_load(S.strm[st] + SP_O_LEN, P.comp + B->len_off + 2ull * j0, b2, &S.mbar[st]);
-    bulk_load(S.strm[st] + SP_O_DEP, P.comp + B->dep_off + 2ull * j0, b2, &S.mbar[st]);
-    bulk_load(S.strm[st] + SP_O_OFF, P.comp + B->off_off + 4ull * j0, b4, &S.mbar[st]);
+    mbar_expect_tx(&S.mbar, 3 * b2 + b4 + (lit_ok ? lbytes : 0u));
+    bulk_load(S.strm, P.comp + F.B.cmd_off + 2ull * j0, b2, &S.mbar);
+    bulk_load(S.strm + SP_O_LEN, P.comp + F.B.len_off + 2ull * j0, b2, &S.mbar);
+    bulk_load(S.strm + SP_O_DEP, P.comp + F.B.dep_off + 2ull * j0, b2, &S.mbar);
+    bulk_load(S.strm + SP_O_OFF, P.comp + F.B.off_off + 4ull * j0, b4, &S.mbar);
+    if (lit_ok && lbytes) bulk_load(S.slit, P.comp + F.B.lit_off + l16, lbytes, &S.mbar);
+}
+// The same slices pulled into L2 ahead of time (the stage is single-buffered: the load proper is issued when the
+// previous tile is done with it and then finds its bytes in L2 instead of DRAM).
+__device__ __forceinline__ void prefetch_tile_l2(const Params& P, uint32_t tile, const TileFetch& F) {
+    const uint32_t j0 = (tile - F.B.tile_base) * TILE;
+    const uint32_t left = F.B.n_seq - j0, n = left < (uint32_t)TILE ? left : (uint32_t)TILE;
+    const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
+    bulk_prefetch_l2(P.comp + F.B.cmd_off + 2ull * j0, b2);
+    bulk_prefetch_l2(P.comp + F.B.len_off + 2ull * j0, b2);
+    bulk_prefetch_l2(P.comp + F.B.dep_off + 2ull * j0, b2);
+    bulk_prefetch_l2(P.comp + F.B.off_off + 4ull * j0, b4);
 }
 
-// ---- register byte-stream writer: appends byte strings to the contiguous piece [start, ..) of the image.
-// Whole words are stored as they fill up, except the thread's FIRST word, which is kept in `first` until the partial
-// word of the preceding thread has been merged in (finish protocol in the kernel).
-struct SpanWriter {
-    unsigned long long acc, first;
-    unsigned long long* img;
-    uint32_t nfill, w, fw;                           // bytes used in acc; image word acc belongs to; first word of the thread
-    __device__ __forceinline__ void init(unsigned long long* img_, uint32_t rel) {
-        img = img_; w = rel >> 3; fw = w; nfill = rel & 7u; acc = 0ull; first = 0ull;
-    }
-    __device__ __forceinline__ void emit(unsigned long long x) {
-        if (w == fw) first = x; else img[w] = x;
-        ++w;
-    }
-    // v: n (1..16) valid bytes, everything above them zero
-    __device__ __forceinline__ void append(V16 v, uint32_t n) {
-        const uint32_t sh = nfill * 8u, tot = nfill + n;
-        unsigned long long w0 = v.lo, c1 = v.hi, c2 = 0ull;
-        if (sh) { w0 = acc | (v.lo << sh); c1 = (v.lo >> (64u - sh)) | (v.hi << sh); c2 = v.hi >> (64u - sh); }
-        if (tot >= 8u) {
-            emit(w0);
-            if (tot >= 16u) { emit(c1); acc = c2; } else acc = c1;
-        } else acc = w0;
-        nfill = tot & 7u;
-    }
-    // n bytes that somebody else writes (a long token, copied later by the whole warp): zeros for now
-    __device__ __forceinline__ void skip(uint32_t n) {
-        const uint32_t tot = nfill + n;
-        if (tot >= 8u) { emit(acc); w += (tot >> 3) - 1u; acc = 0ull; }
-        nfill = tot & 7u;
-    }
-};
-
-__device__ __forceinline__ V16 mask_bytes(V16 v, uint32_t n) {                  // keep the first n (1..16) bytes
-    if (n < 8u) { v.lo &= (1ull << (n * 8u)) - 1ull; v.hi = 0ull; }
-    else if (n < 16u) v.hi &= n == 8u ? 0ull : (1ull << ((n - 8u) * 8u)) - 1ull;
-    return v;
-}
-
-// bytes [sb, sb+16) of the 32-byte pair (wa | wb << 128), sb in 0..15
-__device__ __forceinline__ V16 extract16(uint4 wa, uint4 wb, uint32_t sb) {
-    const unsigned long long a0 = (unsigned long long)wa.x | ((unsigned long long)wa.y << 32), a1 = (unsigned long long)wa.z | ((unsigned long long)wa.w << 32),
-                             b0 = (unsigned long long)wb.x | ((unsigned long long)wb.y << 32), b1 = (unsigned long long)wb.z | ((unsigned long long)wb.w << 32);
-    const unsigned long long x0 = sb < 8u ? a0 : a1, x1 = sb < 8u ? a1 : b0, x2 = sb < 8u ? b0 : b1;
-    const uint32_t s = (sb & 7u) * 8u;
+// bytes [sb, sb+16) of the 24-byte value (x0 | x1 << 64 | x2 << 128), sb in 0..7
+__device__ __forceinline__ V16 extract16(unsigned long long x0, unsigned long long x1, unsigned long long x2, uint32_t sb) {
+    const uint32_t s = sb * 8u;
     V16 v;
     if (s) { v.lo = (x0 >> s) | (x1 << (64u - s)); v.hi = (x1 >> s) | (x2 << (64u - s)); } else { v.lo = x0; v.hi = x1; }
     return v;
 }
 
-constexpr uint32_t SP_SHORT = 16;                    // tokens up to this length go through the thread's registers
+// chain_sync[0] = frontier (blocks 0 .. frontier-1 are completely written); chain_sync[32 + b] = finished tiles of block b
+constexpr uint32_t CH_CNT0 = 32;
 
-__global__ void __launch_bounds__(SP_THREADS, AX_SP_OCC) k_span(Params P, uint32_t depth_hi) {
+template <bool CHAIN>
+__global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t depth_hi) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SpanSmem& S = *reinterpret_cast<SpanSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     if (P.status->fault_flags != 0) return;          // a faulty stream is flagged, not decoded further (uniform: final before this launch)
+    uint32_t tile = blockIdx.x;
+    TileFetch& F = S.fetch;
     if (tid == 0) {
-        mbar_init(&S.mbar[0], 1); mbar_init(&S.mbar[1], 1);
+        mbar_init(&S.mbar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (tile < P.n_tiles) {
+            fetch_step1(P, F, tile); fetch_step2(P, F);
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            issue_tile_loads(P, S, tile, F);
+        }
     }
     __syncthreads();
-    uint32_t tile = blockIdx.x;
-    if (tid == 0 && tile < P.n_tiles) issue_tile_loads(P, S, tile, 0);
     uint32_t n_copied = 0;
-    unsigned long long* const img64 = reinterpret_cast<unsigned long long*>(S.img);
+    uint16_t* const s_cmd = reinterpret_cast<uint16_t*>(S.strm);
+    uint16_t* const s_len = reinterpret_cast<uint16_t*>(S.strm + SP_O_LEN);
+    uint16_t* const s_dep = reinterpret_cast<uint16_t*>(S.strm + SP_O_DEP);
+    uint32_t* const s_off = reinterpret_cast<uint32_t*>(S.strm + SP_O_OFF);
 
     for (uint32_t it = 0; tile < P.n_tiles; ++it, tile += gridDim.x) {
-        const uint32_t st = it & 1u, par = (it >> 1) & 1u;
-        // stage st^1 was last read in iteration it-1, and every thread has passed a __syncthreads since
-        if (tid == 0 && tile + gridDim.x < P.n_tiles) issue_tile_loads(P, S, tile + gridDim.x, st ^ 1u);
-        const uint32_t b = P.tile_blk[tile];
-        const unsigned long long pre = P.tile_state[tile];
-        const BlockDesc* B = P.blocks + b;
-        const uint32_t blk_lo = (uint32_t)B->out_base, tile_base = B->tile_base, n_seq = B->n_seq;
-        const uint8_t* lit = P.comp + B->lit_off;
-        const uint32_t j0 = (tile - tile_base) * TILE, left = n_seq - j0, nt = left < (uint32_t)TILE ? left : (uint32_t)TILE;
-        const uint32_t jt = tid * PRE_ITEMS;
-        // ---- a2: parse from the staged slices
-        mbar_wait(&S.mbar[st], par);
-        Seq8 q;
+        const uint32_t next = tile + gridDim.x;
+        const bool has_next = next < P.n_tiles;
+        if (tid == 0 && has_next) fetch_step1(P, F, next);                 // consumed after the scan below
+        // ---- a2: the tile's slices have landed
+        mbar_wait(&S.mbar, it & 1u);
+        const unsigned long long pre = S.meta.pre;
+        const uint8_t* const lit = S.meta.lit;
+        const uint32_t b = S.meta.b, blk_lo = S.meta.blk_lo, nt = S.meta.nt, blk_tiles = S.meta.blk_tiles;
+        const uint8_t* const lsrc_base = S.meta.lit_ok ? S.slit - S.meta.lit16 : lit;   // byte x of the block's lit[] is lsrc_base[x]
+        const uint32_t A0 = blk_lo + (uint32_t)(pre >> 32);               // absolute start of the tile's span
+        const uint32_t img_org = A0 & ~15u;                               // absolute position of image byte 0
+        // ================= phase S (thread t owns sequences 4t .. 4t+3): a3 scan, token validation
+        const uint32_t jt = tid * SP_PER;
+        uint32_t c4[SP_PER], l4[SP_PER], d4[SP_PER], o4[SP_PER];
         {
-            const uint8_t* sb = S.strm[st];
-            const uint4 z = make_uint4(0u, 0u, 0u, 0u);
-            if (jt < nt)
-                parse8(q, *reinterpret_cast<const uint4*>(sb + 2u * jt), *reinterpret_cast<const uint4*>(sb + SP_O_LEN + 2u * jt),
-                       *reinterpret_cast<const uint4*>(sb + SP_O_DEP + 2u * jt), *reinterpret_cast<const uint4*>(sb + SP_O_OFF + 4u * jt),
-                       *reinterpret_cast<const uint4*>(sb + SP_O_OFF + 4u * jt + 16u), nt - jt);
-            else parse8(q, z, z, z, z, z, 0);
+            uint2 vc = make_uint2(0u, 0u), vl = vc, vd = vc; uint4 vo = make_uint4(0u, 0u, 0u, 0u);
+            if (jt < nt) {
+                vc = *reinterpret_cast<const uint2*>(s_cmd + jt); vl = *reinterpret_cast<const uint2*>(s_len + jt);
+                vd = *reinterpret_cast<const uint2*>(s_dep + jt); vo = *reinterpret_cast<const uint4*>(s_off + jt);
+            }
+            c4[0] = vc.x & 0xFFFFu; c4[1] = vc.x >> 16; c4[2] = vc.y & 0xFFFFu; c4[3] = vc.y >> 16;
+            l4[0] = vl.x & 0xFFFFu; l4[1] = vl.x >> 16; l4[2] = vl.y & 0xFFFFu; l4[3] = vl.y >> 16;
+            d4[0] = vd.x & 0xFFFFu; d4[1] = vd.x >> 16; d4[2] = vd.y & 0xFFFFu; d4[3] = vd.y >> 16;
+            o4[0] = vo.x; o4[1] = vo.y; o4[2] = vo.z; o4[3] = vo.w;
         }
-        // ---- a3: scan of (cmd+len, cmd) packed as (hi, lo) of one u64
         unsigned long long tsum = 0;
+        bool wait_src = false;                       // CHAIN: a match deeper than 1 reads an earlier block
 #pragma unroll
-        for (int k = 0; k < PRE_ITEMS; ++k) tsum += ((unsigned long long)(q.c[k] + q.l[k]) << 32) | q.c[k];
+        for (int k = 0; k < SP_PER; ++k) {
+            if (jt + k >= nt) { c4[k] = 0; l4[k] = 0; }                   // the tail shares its words with nothing: mask
+            tsum += ((unsigned long long)(c4[k] + l4[k]) << 32) | c4[k];
+            if (CHAIN) wait_src |= l4[k] != 0 && o4[k] < blk_lo && d4[k] != 1u;
+        }
         unsigned long long inc = tsum;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -188,162 +242,183 @@ __global__ void __launch_bounds__(SP_THREADS, AX_SP_OCC) k_span(Params P, uint32
             if (lane >= (uint32_t)d) inc += t;
         }
         if (lane == 31) S.warp_sum[warp] = inc;
-        const uint32_t A0 = blk_lo + (uint32_t)(pre >> 32);               // absolute start of the tile's span
-        const uint32_t img_org = A0 & ~15u;                               // absolute position of image byte 0
         if (tid == 0) {
             asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the previous tile's store has read the image
-            S.img_end[st] = A0;
+            S.img_end = A0;
         }
-        __syncthreads();
-        unsigned long long wpre = 0;
-#pragma unroll
-        for (int w = 0; w < SP_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
-        const unsigned long long ex = pre + wpre + (inc - tsum);
-        const uint32_t ts = blk_lo + (uint32_t)(ex >> 32);                // absolute start of this thread's piece
-        const uint32_t te = ts + (uint32_t)(tsum >> 32);
-        const uint32_t lsrc0 = (uint32_t)ex;                              // offset inside the block's lit[]
-        const bool use_img = te - img_org <= SP_IMG;                      // a prefix of the CTA's threads (te is monotone)
+        const bool must_wait = __syncthreads_or(wait_src) != 0;           // barrier 1
         {
-            const uint32_t m = __reduce_max_sync(0xFFFFFFFFu, use_img ? te : 0u);
-            const uint32_t cnt = __popc(__ballot_sync(0xFFFFFFFFu, use_img));
-            if (lane == 0) { if (cnt) atomicMax(&S.img_end[st], m); S.n_img[warp] = cnt; }
+            unsigned long long wpre = 0;
+#pragma unroll
+            for (int w = 0; w < SP_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
+            const unsigned long long ex = pre + wpre + (inc - tsum);
+            uint32_t p = blk_lo + (uint32_t)(ex >> 32), ls = (uint32_t)ex;   // this thread's first token: position, literal offset
+            uint32_t ps[SP_PER], lp[SP_PER];
+            uint32_t bad_src = 0, bad_dep = 0, fit_end = 0;
+#pragma unroll
+            for (int k = 0; k < SP_PER; ++k) {
+                ps[k] = p; lp[k] = ls;
+                const uint32_t mdst = p + c4[k];
+                if (l4[k]) {                                               // token validation (I2, depth range, I3)
+                    if (o4[k] >= mdst || l4[k] < P.min_match) bad_src |= 1u << k;
+                    else if (d4[k] == 0 || d4[k] > (CHAIN ? P.max_depth : depth_hi)) bad_dep |= 1u << k;
+                    else if (CHAIN && o4[k] >= blk_lo && d4[k] != 1u) bad_dep |= 1u << k;   // an in-block source that is not literal
+                }
+                p = mdst + l4[k]; ls += c4[k];
+                if (p - img_org <= SP_IMG) fit_end = p;                   // tokens are monotone: a prefix of the tile fits the image
+            }
+            if (jt < nt) {
+                *reinterpret_cast<uint4*>(S.pos + jt) = make_uint4(ps[0], ps[1], ps[2], ps[3]);
+                *reinterpret_cast<uint4*>(S.lpos + jt) = make_uint4(lp[0], lp[1], lp[2], lp[3]);
+            }
+            if (bad_src | bad_dep) {                                      // a faulty match is flagged and skipped: its bytes stay a hole
+#pragma unroll
+                for (int k = 0; k < SP_PER; ++k) if ((bad_src | bad_dep) & (1u << k)) s_len[jt + k] = 0;
+                if (bad_src) raise_fault(P.status, F_SOURCE, b);
+                if (bad_dep) raise_fault(P.status, F_DEPTH, b);
+            }
+            fit_end = __reduce_max_sync(0xFFFFFFFFu, fit_end);
+            if (lane == 0 && fit_end) atomicMax(&S.img_end, fit_end);
         }
-        SpanWriter W;
-        W.init(img64, ts - img_org);
-        uint32_t p = ts, ls = lsrc0;
-        uint32_t bad = 0;                                                 // bit k: match k is invalid (hole)
-        bool has_long = false;
-        // ---- a6: two batches of four tokens: all gathers of a batch are issued before the first append
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            uint4 wa[4], wb[4];
-            uint32_t pp = p;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int k = 4 * h + i;
-                pp += q.c[k];
-                const uint32_t l = q.l[k];
-                wa[i] = make_uint4(0u, 0u, 0u, 0u); wb[i] = wa[i];
+        if (tid == 0 && has_next) fetch_step2(P, F);                       // (its block index has arrived by now)
+        __syncthreads();                                                  // barrier 2: pos[] / lpos[] / cleared len[] visible
+        // ================= phase L (thread t takes tokens t, t + SP_THREADS, ...; so do phases G and M: a token is handled
+        // by ONE thread from here on, which is why they need no barrier between them).  Needs nothing another block wrote:
+        // literal runs go into the image, and each match is reduced to what the copy needs —
+        //   pos[j]  <- aligned source address (short match) / source address (long match)
+        //   lpos[j] <- info: len (16 bits) | source byte phase (3) | period if the source overlaps, else 0 (4) | in image |
+        //              being copied by this pass | valid
+        //   off[j]  <- match destination
+#pragma unroll 1
+        for (uint32_t j0 = warp * 32u; j0 < nt; j0 += SP_THREADS) {
+            const uint32_t j = j0 + lane;
+            const bool live = j < nt;
+            const uint32_t c = live ? s_cmd[j] : 0u, l = live ? s_len[j] : 0u;
+            const uint32_t ps = live ? S.pos[j] : 0u, lp = live ? S.lpos[j] : 0u;
+            const uint32_t pp = ps + c;
+            const bool in_img = pp + l - img_org <= SP_IMG;
+            if (c && in_img && c <= SP_SHORT) store16(S.img + (ps - img_org), load16(lsrc_base + lp, c), c);
+            uint32_t m = __ballot_sync(0xFFFFFFFFu, c > SP_SHORT && in_img);
+            while (m) {                                                   // long literal runs: the whole warp copies each
+                const int sl = __ffs(m) - 1; m &= m - 1;
+                const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, ps, sl), s2 = __shfl_sync(0xFFFFFFFFu, lp, sl), n2 = __shfl_sync(0xFFFFFFFFu, c, sl);
+                warp_copy(S.img + (d2 - img_org), lit + s2, n2, lane);
+            }
+            if (live) {
+                uint32_t inf = 0, sa = 0;
                 if (l) {
-                    const bool deep = q.dp[k] == depth_hi;
-                    if (q.of[k] >= pp || q.dp[k] == 0 || q.dp[k] > depth_hi) bad |= 1u << k;
-                    else if (l <= SP_SHORT && (use_img || deep)) {
-                        const uint32_t src = deep ? q.of[k] : pp;
-                        const uint32_t dist = pp - q.of[k];
-                        const uint32_t need = (deep && dist < l) ? dist : l;
-                        const uint4* g = reinterpret_cast<const uint4*>(P.out + (src & ~15u));
-                        wa[i] = g[0];
-                        if ((src & 15u) + need > 16u) wb[i] = g[1];
+                    const bool deep = CHAIN || s_dep[j] == depth_hi;
+                    if (in_img || deep) {
+                        const uint32_t of = s_off[j];
+                        const uint32_t src = deep ? of : pp, dist = pp - of;
+                        const bool ovl = deep && dist < l && l <= SP_SHORT;
+                        sa = l <= SP_SHORT ? (src & ~7u) : src;
+                        inf = l | (src & 7u) << 16 | (ovl ? dist : 0u) << 19 | (in_img ? 1u << 23 : 0u) | (deep ? 1u << 24 : 0u) | 1u << 25;
+                        if (deep) ++n_copied;
                     }
                 }
-                pp += l;
-            }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int k = 4 * h + i;
-                const uint32_t c = q.c[k], l = q.l[k];
-                if (c) {                                                  // literal run (rare on compressible data)
-                    if (use_img) {
-                        if (c <= SP_SHORT) W.append(mask_bytes(load16(lit + ls, c), c), c);
-                        else { W.skip(c); has_long = true; }
-                    }
-                    p += c; ls += c;
-                }
-                if (l) {
-                    const bool deep = q.dp[k] == depth_hi, ok = !(bad & (1u << k));
-                    if (ok && deep) ++n_copied;
-                    if (l <= SP_SHORT && ok && (use_img || deep)) {
-                        const uint32_t src = deep ? q.of[k] : p, dist = p - q.of[k];
-                        V16 v = extract16(wa[i], wb[i], src & 15u);
-                        if (deep && dist < l) v = extend_period(v, dist);  // self-overlap: periodic extension (Q3)
-                        v = mask_bytes(v, l);
-                        if (use_img) W.append(v, l); else store16(P.out + p, v, l);
-                    } else {
-                        if (use_img) W.skip(l);
-                        if (ok && (use_img || deep)) has_long = true;
-                    }
-                    p += l;
-                }
+                S.pos[j] = sa; S.lpos[j] = inf; s_off[j] = pp;
             }
         }
-        if (bad) raise_fault(P.status, F_SOURCE, b);
-        // ---- finish protocol: the partial last word of every piece is merged into the first word of the next piece
-        // (segmented OR-scan keyed by image word: pieces shorter than a word chain through several lanes)
-        unsigned long long val = use_img ? W.acc : 0ull;
-        const uint32_t key = use_img ? W.w : KEY_NONE;
-        const bool tiny = use_img && W.w == W.fw;                         // the piece never left its first word
-        if (__any_sync(0xFFFFFFFFu, tiny)) {
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const unsigned long long v2 = __shfl_up_sync(0xFFFFFFFFu, val, d);
-                const uint32_t k2 = __shfl_up_sync(0xFFFFFFFFu, key, d);
-                if (lane >= (uint32_t)d && k2 == key) val |= v2;
-            }
-        }
-        if (lane == 31) { S.tail_val[warp] = val; S.tail_key[warp] = key; }
-        if (lane == 0) S.head_key[warp] = use_img ? W.fw : KEY_NONE;
-        const bool any_long = __syncthreads_or(has_long);                 // barrier A
-        {
-            // what the preceding warps contribute to this warp's first word fw0: the tail of warp-1, and of the warps
-            // before it for as long as a whole warp lies inside that one word
-            const uint32_t fw0 = __shfl_sync(0xFFFFFFFFu, use_img ? W.fw : KEY_NONE, 0);
-            unsigned long long carry = 0ull;
-            if (lane == 0 && use_img) {
-                for (int j = (int)warp - 1; j >= 0; --j) {
-                    if (S.tail_key[j] != fw0) break;
-                    carry |= S.tail_val[j];
-                    if (S.head_key[j] != S.tail_key[j]) break;
+        if (CHAIN && must_wait) {
+            // a7 for strategy CHAIN: every block before this one completely written?  One thread spins on the frontier;
+            // its acquire fence also drops this SM's L1 (CCTL.IVALL), so the loads below see what other SMs wrote.
+            if (tid == 0) {
+                uint32_t v;
+                for (;;) {
+                    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory");
+                    if (v >= b) break;
+                    if (v + 1u < b) __nanosleep(400);                     // not next in line: keep the hot line's queue short
                 }
+                asm volatile("fence.acq_rel.gpu;" ::: "memory");
             }
-            carry = __shfl_sync(0xFFFFFFFFu, carry, 0);
-            if (use_img && key == fw0) val |= carry;                      // lanes whose chain reaches back past lane 0
-            const unsigned long long prev = __shfl_up_sync(0xFFFFFFFFu, val, 1);
-            const unsigned long long chain_in = lane ? prev : carry;      // the preceding piece ends where this one starts
-            uint32_t n_img = 0;
-#pragma unroll
-            for (int w = 0; w < SP_WARPS; ++w) n_img += S.n_img[w];
-            if (use_img && !tiny) img64[W.fw] = W.first | chain_in;
-            if (use_img && tid + 1 == n_img) img64[key] = val;            // last image piece: its (chained) partial word
+            __syncthreads();                                              // barrier 3
         }
-        // ---- long tokens: the whole warp copies each (image mode: into the image; direct mode: depth-D matches only)
-        if (any_long) {
-            __syncthreads();                                              // barrier B: short stores before long copies into the same words
-            uint32_t p2 = ts, ls2 = lsrc0;
+        // ================= phase G: the aligned 8-byte words holding each short match's source travel global -> shared
 #pragma unroll
-            for (int k = 0; k < PRE_ITEMS; ++k) {
-                const uint32_t c = q.c[k], l = q.l[k];
-                uint32_t m = __ballot_sync(0xFFFFFFFFu, use_img && c > SP_SHORT);
+        for (int k = 0; k < SP_PER; ++k) {
+            const uint32_t j = k * SP_THREADS + tid;
+            if (j >= nt) continue;
+            const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
+            if (l == 0 || l > SP_SHORT) continue;
+            const uint32_t per = (inf >> 19) & 15u;
+            const uint32_t span = ((inf >> 16) & 7u) + (per ? per : l);
+            const uint8_t* g = P.out + S.pos[j];
+            cp_async8(&S.x0[j], g);
+            if (span > 8u) cp_async8(&S.x1[j], g + 8);
+            if (span > 16u) cp_async8(&S.x2[j], g + 16);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        if (tid == 0 && has_next) prefetch_tile_l2(P, next, F);
+        // ================= phase M: a6, every match into the image (or, beyond its capacity, straight to global memory).
+        // The thread's four tokens are unrolled so that their dependent shift / store chains interleave.
+        bool any_long = false;
+#pragma unroll
+        for (int k = 0; k < SP_PER; ++k) {
+            const uint32_t j = k * SP_THREADS + tid;
+            if (j >= nt) continue;
+            const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
+            any_long |= l > SP_SHORT;
+            if (l != 0 && l <= SP_SHORT) {
+                const uint32_t pp = s_off[j], per = (inf >> 19) & 15u;
+                V16 v = extract16(S.x0[j], S.x1[j], S.x2[j], (inf >> 16) & 7u);
+                if (per) v = extend_period(v, per);                        // self-overlap: periodic extension (Q3)
+                store16((inf >> 23) & 1u ? S.img + (pp - img_org) : P.out + pp, v, l);
+            }
+        }
+        if (__any_sync(0xFFFFFFFFu, any_long)) {                          // long matches: the whole warp copies each
+#pragma unroll 1
+            for (uint32_t j0 = warp * 32u; j0 < nt; j0 += SP_THREADS) {
+                const uint32_t j = j0 + lane;
+                const bool live = j < nt;
+                const uint32_t inf = live ? S.lpos[j] : 0u, l = inf & 0xFFFFu;
+                const uint32_t pp = live ? s_off[j] : 0u, sa = live ? S.pos[j] : 0u;
+                uint32_t m = __ballot_sync(0xFFFFFFFFu, l > SP_SHORT);
                 while (m) {
                     const int sl = __ffs(m) - 1; m &= m - 1;
-                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, p2, sl), s2 = __shfl_sync(0xFFFFFFFFu, ls2, sl), n2 = __shfl_sync(0xFFFFFFFFu, c, sl);
-                    warp_copy(S.img + (d2 - img_org), lit + s2, n2, lane);
-                }
-                p2 += c; ls2 += c;
-                const bool deep = q.dp[k] == depth_hi;
-                m = __ballot_sync(0xFFFFFFFFu, l > SP_SHORT && !(bad & (1u << k)) && (use_img || deep));
-                while (m) {
-                    const int sl = __ffs(m) - 1; m &= m - 1;
-                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, p2, sl), o2 = __shfl_sync(0xFFFFFFFFu, q.of[k], sl), n2 = __shfl_sync(0xFFFFFFFFu, l, sl);
-                    const bool dp2 = __shfl_sync(0xFFFFFFFFu, (uint32_t)deep, sl) != 0, im2 = __shfl_sync(0xFFFFFFFFu, (uint32_t)use_img, sl) != 0;
+                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, pp, sl), o2 = __shfl_sync(0xFFFFFFFFu, sa, sl),
+                                   n2 = __shfl_sync(0xFFFFFFFFu, l, sl), f2 = __shfl_sync(0xFFFFFFFFu, inf, sl);
+                    const bool im2 = (f2 >> 23) & 1u;
                     uint8_t* dst = im2 ? S.img + (d2 - img_org) : P.out + d2;
-                    if (dp2) warp_match(dst, P.out + o2, n2, d2 - o2, false, lane);
-                    else warp_copy(dst, P.out + d2, n2, lane);              // (image mode only) its own bytes
+                    if ((f2 >> 24) & 1u) warp_match(dst, P.out + o2, n2, d2 - o2, !im2, lane);
+                    else warp_copy(dst, P.out + o2, n2, lane);             // (SPAN, image mode only) its own bytes: o2 == d2
                 }
-                p2 += l;
             }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy image writes -> visible to the bulk store
-        __syncthreads();                                                  // barrier C
-        // ---- write the image out: 16-byte chunks by one bulk TMA store, the partial chunks at both ends by byte stores
-        {
-            const uint32_t E = S.img_end[st];
+        __syncthreads();                                                  // barrier 4: image complete, stage free
+        if (tid < 32u) {
+            // ---- write the image out: 16-byte chunks by one bulk TMA store, the partial chunks at both ends by byte stores
+            const uint32_t E = S.img_end;
             const uint32_t c0 = (A0 + 15u) & ~15u, c1 = E & ~15u;
             if (tid == 0 && c1 > c0) bulk_store(P.out + c0, S.img + (c0 - img_org), c1 - c0);
+            // the next tile's slices start travelling while this tile's image is stored
+            if (tid == 0 && has_next) issue_tile_loads(P, S, next, F);
             const uint32_t he = c0 < E ? c0 : E;                          // head bytes [A0, he)
             if (tid < 16u && A0 + tid < he) P.out[A0 + tid] = S.img[A0 + tid - img_org];
-            if (tid >= 16u && tid < 32u && c1 >= c0) {                    // tail bytes [c1, E)
+            if (tid >= 16u && c1 >= c0) {                                 // tail bytes [c1, E)
                 const uint32_t a = c1 + (tid - 16u);
                 if (a < E) P.out[a] = S.img[a - img_org];
+            }
+            if (CHAIN) {
+                // publish: the tile's bytes (bulk store complete, head / tail / direct stores ordered by barrier 4 and the
+                // warp barrier) happen before the release-add; the tile that completes block b moves the frontier, in
+                // block order (blocks whose tiles never had to wait may finish early).
+                if (tid == 0) {
+                    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+                    asm volatile("fence.proxy.async;" ::: "memory");
+                }
+                __syncwarp();
+                if (tid == 0) {
+                    uint32_t old;
+                    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
+                    if (old + 1u == blk_tiles) {
+                        uint32_t v;
+                        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory"); } while (v < b);
+                        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(P.chain_sync), "r"(b + 1u) : "memory");
+                    }
+                }
             }
         }
     }
@@ -356,19 +431,36 @@ __global__ void __launch_bounds__(SP_THREADS, AX_SP_OCC) k_span(Params P, uint32
 size_t span_smem_bytes() { return sizeof(SpanSmem); }
 
 cudaError_t span_configure() {
-    return cudaFuncSetAttribute(k_span, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
+    cudaError_t e = cudaFuncSetAttribute(k_span<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_span<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
 }
 
 int span_max_ctas_per_sm() {
-    int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_span, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
-    return n;
+    int n = 0, m = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_span<false>, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m, k_span<true>, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
+    return n < m ? n : m;
 }
 
 void launch_span(const Params& P, uint32_t depth_hi, int grid, cudaStream_t st) {
     if (!P.n_tiles) return;
     const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
-    k_span<<<g, SP_THREADS, sizeof(SpanSmem), st>>>(P, depth_hi);
+    k_span<false><<<g, SP_THREADS, sizeof(SpanSmem), st>>>(P, depth_hi);
 }
+
+// Strategy CHAIN: every tile of the grid must be resident (a tile spins on the frontier that lower tiles advance), so the
+// launch is cooperative and the grid at most n_sm x occupancy; frontier and per-block counts start from zero.
+cudaError_t launch_chain(const Params& P, int grid, cudaStream_t st) {
+    if (!P.n_tiles) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(P.chain_sync, 0, sizeof(uint32_t) * (CH_CNT0 + (size_t)P.n_blocks), st);
+    if (e != cudaSuccess) return e;
+    uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles, zero = 0;
+    Params p = P;
+    void* args[] = {&p, &zero};
+    return cudaLaunchCooperativeKernel((const void*)k_span<true>, dim3(g), dim3(SP_THREADS), args, sizeof(SpanSmem), st);
+}
+
+size_t chain_sync_words(uint32_t n_blocks) { return CH_CNT0 + (size_t)n_blocks; }
 
 }  // namespace ax

@@ -9,10 +9,11 @@
 
 namespace ax {
 
-constexpr int TS_WARPS = PRE_THREADS / 32;
+constexpr int TS_THREADS = 256;
+constexpr int TS_WARPS = TS_THREADS / 32;
 constexpr uint32_t TS_CHUNK = 1024;
 
-__global__ void __launch_bounds__(PRE_THREADS) k_tilesum(Params P) {
+__global__ void __launch_bounds__(TS_THREADS) k_tilesum(Params P) {
     __shared__ unsigned long long s_tot[TS_CHUNK];
     __shared__ unsigned long long s_carry;
     if (P.status->fault_flags & F_INDEX) return;         // the block index itself is inconsistent: nothing below is safe
@@ -70,7 +71,7 @@ __global__ void __launch_bounds__(PRE_THREADS) k_tilesum(Params P) {
 }
 
 void launch_tilesum(const Params& P, int grid, cudaStream_t st) {
-    if (P.n_blocks) k_tilesum<<<(uint32_t)grid < P.n_blocks ? grid : P.n_blocks, PRE_THREADS, 0, st>>>(P);
+    if (P.n_blocks) k_tilesum<<<(uint32_t)grid < P.n_blocks ? grid : P.n_blocks, TS_THREADS, 0, st>>>(P);
 }
 
 }  // namespace ax

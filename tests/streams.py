@@ -154,3 +154,31 @@ def random_blocks(rng: np.random.Generator, block_size: int, n_blocks: int, *, l
             p += mlen
         blocks.append(blk)
     return blocks
+
+
+def flatten_blocks(blocks, block_size):
+    """Make a hand-built description satisfy invariant I3 (after chain flattening no match reads a byte
+    another match of its own block produced) without changing the decoded bytes: a match whose effective source range
+    touches a match-written byte of its own block is replaced by literals of the same bytes."""
+    exp = py_decode(blocks)
+    out, p = [], 0
+    for blk in blocks:
+        lo = p
+        is_match = bytearray(block_size + 1)                      # per byte of this block: written by a match
+        nb = []
+        for lit, mlen, off in blk:
+            p += len(lit)
+            if mlen:
+                se = min(off + mlen, p)
+                if any(is_match[i - lo] for i in range(max(off, lo), se)):
+                    nb.append((lit + exp[p:p + mlen], 0, 0))
+                else:
+                    nb.append((lit, mlen, off))
+                    for i in range(p, p + mlen):
+                        is_match[i - lo] = 1
+                p += mlen
+            else:
+                nb.append((lit, 0, 0))
+        out.append(nb)
+    assert py_decode(out) == exp
+    return out

@@ -8,7 +8,7 @@ import pytest
 import oracle
 import workloads
 import paper_2606_04268_b200 as ax
-from streams import build_stream, py_decode, py_depths, random_blocks
+from streams import build_stream, flatten_blocks, py_decode, py_depths, random_blocks
 
 pytestmark = pytest.mark.gpu
 
@@ -19,6 +19,21 @@ ALL_STRATS = STRATS + [ax.WAVES_SPAN]                                 # + last d
 def span_ok(comp):
     """Strategy SPAN needs at least one match depth (header offset 40: max_depth)."""
     return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) >= 1
+
+
+def chain_ok(comp):
+    """Strategy CHAIN needs the header's FLATTENED flag (offset 12, bit 0): invariant I3."""
+    return bool(int(np.frombuffer(comp[12:16].tobytes(), "<u4")[0]) & 1)
+
+
+def passes_ok(comp):
+    """Strategy PASSES runs one streaming pass per depth and accepts at most 16 of them."""
+    return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) <= 16
+
+
+def strats_for(comp):
+    return STRATS + ([ax.WAVES_SPAN] if span_ok(comp) else []) + ([ax.WAVES_CHAIN] if chain_ok(comp) else []) + \
+        ([ax.WAVES_PASSES] if passes_ok(comp) else [])
 
 
 def gpu_decode(comp, strategy=0, check=True):
@@ -36,8 +51,8 @@ def gpu_decode(comp, strategy=0, check=True):
 def assert_parity(comp, raw=None, strategies=STRATS):
     want = oracle.decode(comp)
     rep = oracle.validate(comp)
-    if strategies is STRATS and span_ok(comp):
-        strategies = ALL_STRATS
+    if strategies is STRATS:
+        strategies = strats_for(comp)
     for s in strategies:
         got, st = gpu_decode(comp, s)
         assert got.size == want.size
@@ -81,9 +96,9 @@ def test_periodic_overlap(k, n):
     pat = bytes((65 + i) % 251 for i in range(k))
     for lead in (b"", b"xy", b"0123456789abcde"):                               # vary destination alignment
         blocks = [[(lead + pat, n, len(lead))]]
-        s = build_stream(blocks, 1 << 17)
+        s = build_stream(blocks, 1 << 17, flags=5)
         exp = lead + (pat * (n // k + 2))[:k + n]
-        for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_SPAN, ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, strat
 
@@ -98,8 +113,8 @@ def test_long_copies_all_alignments():
             lit = rng.integers(0, 256, 17 + da, dtype=np.uint8).tobytes()
             seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
     blocks = [seqs]
-    s = build_stream(blocks, 1 << 20)
-    for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+    s = build_stream(blocks, 1 << 20, flags=5)                                  # every source is literal: I3 holds
+    for strat in (ax.WAVES_SPAN, ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
         got, _ = gpu_decode(s, strat)
         assert got.tobytes() == py_decode(blocks), strat
 
@@ -112,7 +127,7 @@ def test_fuzz_streams(bs, nb, seed):
         blocks = random_blocks(rng, bs, nb, max_len=40 if bs < 4096 else 300, max_lit=12 if bs < 4096 else 40)
         s = build_stream(blocks, bs, min_match=1)
         exp = py_decode(blocks)
-        for strat in (ALL_STRATS if span_ok(s) else STRATS):
+        for strat in strats_for(s):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, it, strat)
 
@@ -165,7 +180,7 @@ def test_phases_and_replay():
     from paper_2606_04268_b200.torch_io import Decoder
     raw = workloads.generate("text", 2 << 20, 9)
     comp = oracle.encode(raw, depth_limit=4)
-    for strat in ALL_STRATS:
+    for strat in ALL_STRATS + [ax.WAVES_CHAIN, ax.WAVES_PASSES]:
         d = Decoder(comp, 0, strat)
         d.run(ax.PHASE_PRE)
         d.run(ax.PHASE_MATCH)
@@ -242,7 +257,7 @@ def test_device_faults_are_flagged_not_fatal():
         t[off:off + len(vals)] = np.frombuffer(bytes(vals), np.uint8)
         return t
     assert run(s)["rc"] == 0
-    for strat in ALL_STRATS:
+    for strat in ALL_STRATS + [ax.WAVES_CHAIN, ax.WAVES_PASSES]:
         st = run(mut(po, [9]), strat)                         # cmd[0] 8 -> 9: block no longer sums
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_BLOCK_SUM and st["fault_block"] == 0
         st = run(mut(po + 48 + 4, [200]), strat)              # off[1] >= mdst
@@ -256,7 +271,7 @@ def test_device_faults_are_flagged_not_fatal():
     two = build_stream([[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]], 32)   # depths 1,2,1
     t = two.copy()
     t[po + 32 + 2] = 1                                        # dep[1] 2 -> 1: counts disagree with the histogram
-    for strat in [0] + ALL_STRATS:
+    for strat in [0] + ALL_STRATS + [ax.WAVES_PASSES]:
         st = run(t, strat)
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
 
@@ -337,9 +352,94 @@ def test_fuzz_shallow_streams_span(seed):
             nblocks.append(nb_)
         assert py_decode(nblocks) == exp
         s = build_stream(nblocks, bs, min_match=1)
-        for strat in (ax.WAVES_SPAN, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_SPAN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, strat)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_fuzz_flattened_streams_chain(seed):
+    """Encoder-free fuzz of strategy CHAIN: random streams made to satisfy I3 (tests/streams.py flatten_blocks), so
+    chains run ACROSS blocks only — arbitrary depths, random overlaps, sources straddling tiles and blocks, blocks of
+    one or many tiles, a short last block."""
+    rng = np.random.default_rng(1300 + seed)
+    for bs, nb in ((64, 40), (4096, 9), (1 << 16, 4), (1 << 18, 3)):
+        blocks = flatten_blocks(random_blocks(rng, bs, nb, max_len=60 if bs < 4096 else 400, max_lit=12 if bs < 4096 else 60,
+                                              p_match=0.7), bs)
+        exp = py_decode(blocks)
+        s = build_stream(blocks, bs, flags=5, min_match=1)
+        for strat in (ax.WAVES_CHAIN, ax.WAVES_LAUNCH):
+            got, st = gpu_decode(s, strat)
+            assert got.tobytes() == exp, (bs, nb, seed, strat)
+    # I3 broken under a FLATTENED header (an in-block source that a match produced): flagged, not decoded
+    bad = [[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]]
+    got, st = gpu_decode(build_stream(bad, 32, flags=5), ax.WAVES_CHAIN, check=False)
+    assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
+
+
+def test_chain_needs_flattened_flag():
+    s = build_stream([[(b"abcdefgh", 8, 0)]], 32)               # flags = HAS_DEP only
+    p = ax.Plan(s.ctypes.data, s.size, 0)
+    with pytest.raises(ax.AceapexError):
+        p.set_strategy(ax.WAVES_CHAIN)
+    p.close()
+
+
+def test_understated_depth_is_undefined_but_in_bounds():
+    """dep[] is trusted for scheduling (include/aceapex.h, docs/FORMAT.md "Trust").  A stream whose dep[]
+    understates a depth, with a histogram to match, is rejected by the oracle validator (I4); the GPU library raises no
+    fault, stays inside its buffers, and its bytes are undefined — the documented limitation, pinned here."""
+    import torch
+    seqs = [[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]]            # true depths 1, 2, 1
+    s = build_stream(seqs, 32, deps=[[1, 1, 1]])
+    with pytest.raises(oracle.OracleError) as e:
+        oracle.validate(s)
+    assert e.value.name == "E_I4"
+    G = 4096
+    for strat in STRATS + [ax.WAVES_SPAN, ax.WAVES_PASSES]:
+        p = ax.Plan(s.ctypes.data, s.size, 0)
+        p.set_strategy(strat)
+        cd = torch.from_numpy(s).cuda()
+        ob, sb = p.out_bytes, (p.scratch_bytes + 255) & ~255
+        big_o = torch.full((G + ob + G,), 0xEE, dtype=torch.uint8, device="cuda")
+        big_s = torch.full((G + sb + G,), 0xEE, dtype=torch.uint8, device="cuda")
+        p.decode(cd.data_ptr(), big_o.data_ptr() + G, ob, big_s.data_ptr() + G, sb, ax.PHASE_ALL, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        assert p.stats(big_s.data_ptr() + G, check=False)["rc"] == 0
+        assert bool((big_o[:G] == 0xEE).all()) and bool((big_o[G + ob:] == 0xEE).all())
+        assert bool((big_s[:G] == 0xEE).all()) and bool((big_s[G + sb:] == 0xEE).all())
+        p.close()
+
+
+def test_adjacent_merges_and_plain_stores_in_one_wave():
+    """within one wave, short non-overlapping matches are OR-merged as whole 8-byte words (red.or.b64) while
+    overlapping short matches and long matches use plain 1..16-byte stores; neighbours of both kinds share 8-byte words.
+    Many such neighbours, every alignment, one wave: the bytes must come out right (the L2 applies reductions and byte-
+    enabled stores to disjoint bytes of a word independently — DESIGN.md 6.1)."""
+    rng = np.random.default_rng(77)
+    base = rng.integers(0, 256, 600, dtype=np.uint8).tobytes()
+    seqs = [(base, 0, 0)]
+    for i in range(3000):
+        kind = i % 3
+        if kind == 0:
+            seqs.append((b"", int(rng.integers(4, 17)), int(rng.integers(0, 500))))          # simple: merged
+        elif kind == 1:
+            seqs.append((bytes([65 + i % 20]), int(rng.integers(5, 30)), 0))                 # placeholder, fixed below
+        else:
+            seqs.append((b"", int(rng.integers(33, 90)), int(rng.integers(0, 400))))         # long: warp copy
+    # kind 1 becomes a self-overlapping short match: source = the literal byte just before it (period 1)
+    pos, fixed = 0, []
+    for lit, ml, off in seqs:
+        pos += len(lit)
+        fixed.append((lit, ml, pos - 1) if (len(lit) == 1 and ml) else (lit, ml, off))
+        pos += ml
+    blocks = [fixed]
+    s = build_stream(blocks, 1 << 20, flags=5)                                               # every source is a literal: one wave
+    exp = py_decode(blocks)
+    for strat in (ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT, ax.WAVES_PASSES, ax.WAVES_CHAIN):
+        for _ in range(3):
+            got, st = gpu_decode(s, strat)
+            assert st["max_depth"] == 1 and got.tobytes() == exp, strat
 
 
 def test_guard_bands_all_strategies():
@@ -353,7 +453,7 @@ def test_guard_bands_all_strategies():
     for kind, n, kw in cases:
         raw = workloads.generate(kind, n, 77)
         comp = oracle.encode(raw, **kw)
-        for strat in (ALL_STRATS if span_ok(comp) else STRATS):
+        for strat in strats_for(comp):
             p = ax.Plan(comp.ctypes.data, comp.size, 0)
             p.set_strategy(strat)
             cd = torch.from_numpy(comp).cuda()
@@ -391,7 +491,7 @@ def test_sparse_depths_empty_waves():
         deps2, _ = py_depths(nblocks, bs)
         doubled = [[2 * d for d in dd] for dd in deps2]
         s = build_stream(nblocks, bs, deps=doubled, min_match=1)
-        for strat in [0] + ALL_STRATS:
+        for strat in [0] + ALL_STRATS + [ax.WAVES_PASSES]:
             got, st = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, strat)
             assert st["max_depth"] % 2 == 0

@@ -242,6 +242,26 @@ def test_malformed_streams_rejected():
 
 
 # ---------------------------------------------------------------- generators are pinned by checksum
+GEN_SHA256_1MIB = {   # docs/WORKLOADS.md: SHA-256 (first 32 hex digits) of the first MiB of each BASELINE config's generator
+    "synth4m": "e7fa8a03e69a46a24ae67c373dc440aa",
+    "text256m": "e9dc67a497379fe02db0cc26cfa8438f",
+    "fastq1g": "27f782f45a4cb36c2a25834aad865f9c",
+    "text1g_d4": "e9dc67a497379fe02db0cc26cfa8438f",
+    "stress2g": "5fc6eaa5080fbd29d8bc5771414ceb5a",
+}
+
+
+def test_generators_pinned_by_checksum():
+    """generator parameters are frozen in docs/WORKLOADS.md and pinned by a checksum of each output.  The
+    generators are prefix-stable, so the first MiB pins the recipe of the full-size configs too."""
+    import hashlib
+    for name, want in GEN_SHA256_1MIB.items():
+        a = workloads.config_bytes(name, 1 << 20)
+        assert hashlib.sha256(a.tobytes()).hexdigest()[:32] == want, name
+        b = workloads.config_bytes(name, (1 << 20) + 4321)
+        assert np.array_equal(a, b[:1 << 20]), f"{name}: not prefix-stable"
+
+
 def test_generators_deterministic():
     a = workloads.generate("text", 100_000, 11)
     b = workloads.generate("text", 100_000, 11)
@@ -253,3 +273,21 @@ def test_generators_deterministic():
     fq = workloads.generate("fastq", 2000, 1).tobytes().split(b"\n")
     assert fq[0].startswith(b"@SIM:") and fq[2] == b"+" and len(fq[1]) == 150 == len(fq[3])
     assert set(fq[1]) <= set(b"ACGTN")
+
+
+# ---------------------------------------------------------------- the oracle under ASan + UBSan
+def test_oracle_under_sanitizers(tmp_path):
+    """Every oracle entry point on BASELINE config 0 (synth4m: 4 blocks of 1 MB) in a build with
+    -fsanitize=address,undefined: tests/asan_driver.c includes oracle/aceapex_oracle.c as is."""
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe = str(tmp_path / "asan_driver")
+    subprocess.check_call(["gcc", "-O1", "-g", "-std=gnu11", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-pthread",
+                           os.path.join(root, "tests", "asan_driver.c"), "-o", exe])
+    raw = workloads.config_bytes("synth4m")
+    f = tmp_path / "synth4m.raw"
+    raw.tofile(f)
+    r = subprocess.run([exe, str(f), str(1 << 20)], capture_output=True, text=True, timeout=600,
+                       env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("ok") == 3
