@@ -38,7 +38,7 @@ WORKLOADS = {
 }
 TARGETS = ["fastq1g", "text1g_d4"]      # BASELINE.json: "the 1 GB text-like and FASTQ-like workloads"; the first is the headline
 BASE_SEED = 260604268
-STRATEGIES = {"launch": 1, "graph": 2, "persistent": 3, "span": 4, "chain": 5, "passes": 6}
+STRATEGIES = {"launch": 1, "graph": 2, "persistent": 3, "passes": 4, "chain": 5}
 PAPER_CONTEXT = {"h100_match_phase_gbs": {"enwik9": 44.0, "fastq": 20.3, "enwik9_depth10": 77.2},
                  "source": "PAPER.md:187-188, :206 (one H100 SXM; context, not the target)"}
 
@@ -403,7 +403,8 @@ def measure(name, args, env) -> dict:
     cnt, byt = plan.depth_hist()
     waves = [c for c in cnt[1:]]
     strat = ax.STRATEGY_NAMES[st["strategy"]]
-    kernel = {"span": "k_waves (depths 1..D-1, one launch each) + k_span (depth D: one streaming pass over the token stream)",
+    kernel = {"chain": "k_chain (every match in one pass over the token stream, tiles ordered by per-block completion counts)",
+              "passes": "k_pass (one streaming pass over the token stream per depth)",
               "persistent": "k_waves (all match waves of one step in one cooperative launch, grid barrier per depth)"}.get(
                   strat, "k_waves (one launch per depth)")
     tr = ncu_traffic(name) if args.size_mb is None and not args.enc_override else None
@@ -493,7 +494,7 @@ def main():
     ap.add_argument("--workload", default=None, choices=sorted(WORKLOADS),
                     help="default: both TARGET configs (fastq1g = headline, text1g_d4 under `targets`)")
     ap.add_argument("--size-mb", type=int, default=None, help="development override of the workload size")
-    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent", "span", "chain", "passes"])
+    ap.add_argument("--strategy", default="auto", choices=["auto", "launch", "graph", "persistent", "passes", "chain"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--flatten", type=int, default=None, choices=[0, 1], help="encoder override (stress sweep): chain flattening")
     ap.add_argument("--depth-limit", type=int, default=None, help="encoder override (stress sweep): depth limit D, 0 = unlimited")

@@ -54,16 +54,13 @@ enum {
     ACEAPEX_WAVES_LAUNCH = 1,     /* wave lists; one kernel launch per depth on the caller's stream          */
     ACEAPEX_WAVES_GRAPH = 2,      /* the same launches replayed from a cached CUDA graph       */
     ACEAPEX_WAVES_PERSISTENT = 3, /* wave lists; one cooperative kernel, grid barrier between depths         */
-    ACEAPEX_WAVES_SPAN = 4,       /* shallow streams whose last depth holds most matches (depth-limited encoder,
-                                     PAPER.md:228): depths 1 .. D-1 through wave lists, depth D by one streaming
-                                     pass over the token stream that writes the whole output once (k_span)   */
-    ACEAPEX_WAVES_PASSES = 6,     /* shallow streams (max_depth <= 16, e.g. the depth-limited encoder of PAPER.md:228): no wave
+    ACEAPEX_WAVES_PASSES = 4,     /* shallow streams (max_depth <= 16, e.g. the depth-limited encoder of PAPER.md:228): no wave
                                      lists; the token stream is re-parsed once per depth, pass p copying the matches with
                                      dep == p (k_pass).  E_ARG from aceapex_set_strategy if max_depth > 16          */
     ACEAPEX_WAVES_CHAIN = 5       /* FLATTENED streams only (after chain flattening no match reads a byte
                                      another match of its own block produced): no wave lists; ONE pass over the token
                                      stream in block order copies every match, a tile waiting until all earlier blocks
-                                     are written (k_span<CHAIN>).  E_ARG from aceapex_set_strategy if the header's
+                                     are written (k_chain).  E_ARG from aceapex_set_strategy if the header's
                                      FLATTENED flag is clear                                                    */
 };
 

@@ -13,14 +13,14 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libaceapex.so")
-_SOURCES = ["k_index.cu", "k_tilesum.cu", "k_pre.cu", "k_match.cu", "k_pass.cu", "k_span.cu", "api.cu"]
+_SOURCES = ["k_index.cu", "k_tilesum.cu", "k_pre.cu", "k_match.cu", "k_pass.cu", "k_chain.cu", "api.cu"]
 _HEADERS = [os.path.join(_CSRC, "common.cuh"), os.path.join(_CSRC, "copy.cuh"), os.path.join(os.path.dirname(_HERE), "include", "aceapex.h")]
 
 OK = 0
 E_MAGIC, E_VERSION, E_TRUNCATED, E_HEADER, E_CAPACITY, E_ALIGN, E_CUDA, E_ARG, E_STREAM, E_NOMEM = range(-1, -11, -1)
 PHASE_PRE, PHASE_MATCH, PHASE_ALL = 1, 2, 3
-WAVES_AUTO, WAVES_LAUNCH, WAVES_GRAPH, WAVES_PERSISTENT, WAVES_SPAN, WAVES_CHAIN, WAVES_PASSES = 0, 1, 2, 3, 4, 5, 6
-STRATEGY_NAMES = {0: "auto", 1: "launch", 2: "graph", 3: "persistent", 4: "span", 5: "chain", 6: "passes"}
+WAVES_AUTO, WAVES_LAUNCH, WAVES_GRAPH, WAVES_PERSISTENT, WAVES_PASSES, WAVES_CHAIN = 0, 1, 2, 3, 4, 5
+STRATEGY_NAMES = {0: "auto", 1: "launch", 2: "graph", 3: "persistent", 4: "passes", 5: "chain"}
 F_BLOCK_SUM, F_SOURCE, F_DEPTH, F_PLACEHOLDER, F_INDEX = 1, 2, 4, 8, 16
 
 EXPORTS = ["aceapex_plan", "aceapex_raw_bytes", "aceapex_out_bytes", "aceapex_scratch_bytes", "aceapex_set_strategy",

@@ -23,9 +23,8 @@ int match_max_ctas_per_sm();
 cudaError_t waves_configure();
 cudaError_t launch_wave(const Params& P, uint32_t depth, uint32_t n_entries, int max_grid, cudaStream_t st);
 cudaError_t launch_waves_persistent(const Params& P, uint32_t d_first, uint32_t d_last, int grid, cudaStream_t st);
-cudaError_t span_configure();
-int span_max_ctas_per_sm();
-void launch_span(const Params& P, uint32_t depth_hi, int grid, cudaStream_t st);
+cudaError_t chain_configure();
+int chain_max_ctas_per_sm();
 cudaError_t launch_chain(const Params& P, int grid, cudaStream_t st);
 size_t chain_sync_words(uint32_t n_blocks);
 }  // namespace ax
@@ -42,9 +41,9 @@ struct aceapex_plan_s {
     uint32_t flags, block_size, n_blocks, min_match, depth_limit, max_depth;
     uint64_t raw_size, total_seq, total_lit, comp_bytes, n_match;
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
-    uint32_t n_tiles;
+    uint32_t n_tiles_list, n_tiles_stream;          // tiles at TILE_LIST / TILE_STREAM sequences per tile
     // device facts
-    int device, n_sm, pre_grid, match_ctas_per_sm, span_grid, pass_grid;
+    int device, n_sm, pre_grid, match_ctas_per_sm, chain_grid, pass_grid;
     // scratch layout (byte offsets)
     size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_chain, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
@@ -76,23 +75,29 @@ extern "C" const char* aceapex_strerror(int code) {
     }
 }
 
-// Wave strategy = the cheapest of three cost estimates built from the header (sequences, matches, depths with matches)
-// and per-unit costs measured on B200 (picoseconds per sequence / match, microseconds per wave):
-//   PASSES      literal pass 6.1 ps/seq + per depth one streaming pass 4.0 ps/seq (+ ~3 us launch) + 8.8 ps per match copied
-//   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5 us + 21 ps per match copied from a list
-//   PERSISTENT  the same lists, one cooperative kernel: ~2.8 us of grid barrier + fence drain per depth instead of a launch
-// PASSES is limited to PASS_MAX_DEPTH waves.  SPAN and CHAIN (k_span) are never chosen here: measured slower than the
-// above on every BASELINE config; they stay selectable through aceapex_set_strategy.
+// Wave strategy = the cheapest of four cost estimates built from the header (sequences, matches, blocks, depths with
+// matches) and per-unit costs measured on B200 (picoseconds per sequence / match, microseconds per step):
+//   PASSES      literal pass 6.1 ps/seq + per depth one streaming pass 3.6 ps/seq (+ ~3 us launch) + 8.8 ps per match copied
+//   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5.5 us + 21 ps per match copied from a list
+//   PERSISTENT  the same lists, one cooperative kernel: ~4 us of grid barrier + fence drain + straggler wait per depth
+//   CHAIN       (FLATTENED streams only) literal pass 3.1 ps/seq, then one pass whose time is the larger of the block chain
+//               (one ~7.1 us hop per 1 MB block) and its issue-bound throughput (26 ps/seq)
+// PASSES is limited to PASS_MAX_DEPTH waves.
 static int choose_strategy(const aceapex_plan_t* p) {
     if (p->max_depth == 0) return ACEAPEX_WAVES_LAUNCH;
     double waves = 0;
     for (uint32_t d = 1; d <= p->max_depth; ++d) waves += p->hist_cnt[d] != 0;
     const double seq = (double)p->total_seq, m = (double)p->n_match;
     const double t_lists = 14.5e-6 * seq + 21e-6 * m;                           // microseconds
-    const double t_launch = t_lists + 5.0 * waves, t_persist = t_lists + 2.8 * waves + 8.0;
-    const double t_passes = p->max_depth <= PASS_MAX_DEPTH ? 6.1e-6 * seq + p->max_depth * (4.0e-6 * seq + 3.0) + 8.8e-6 * m : 1e300;
-    if (t_passes <= t_launch && t_passes <= t_persist) return ACEAPEX_WAVES_PASSES;
-    return t_launch <= t_persist ? ACEAPEX_WAVES_LAUNCH : ACEAPEX_WAVES_PERSISTENT;
+    const double t_launch = t_lists + 5.5 * waves, t_persist = t_lists + 4.0 * waves + 8.0;
+    const double t_passes = p->max_depth <= PASS_MAX_DEPTH ? 6.1e-6 * seq + p->max_depth * (3.6e-6 * seq + 3.0) + 8.8e-6 * m : 1e300;
+    const double hop = 7.1 * p->n_blocks, thr = 26e-6 * seq;
+    const double t_chain = (p->flags & FLAG_FLATTENED) ? 3.1e-6 * seq + (hop > thr ? hop : thr) + 10.0 : 1e300;
+    int best = ACEAPEX_WAVES_LAUNCH; double t = t_launch;
+    if (t_persist < t) { best = ACEAPEX_WAVES_PERSISTENT; t = t_persist; }
+    if (t_passes < t) { best = ACEAPEX_WAVES_PASSES; t = t_passes; }
+    if (t_chain < t) { best = ACEAPEX_WAVES_CHAIN; t = t_chain; }
+    return best;
 }
 
 extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device, aceapex_plan_t** out) {
@@ -119,17 +124,17 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (meta_p > comp_bytes) { rc = ACEAPEX_E_TRUNCATED; break; }
         const uint8_t* dir = c + HDR_BYTES;
         const uint8_t* hist = dir + DIR_BYTES * nb;
-        uint64_t prev_end = meta_p, ts = 0, tl = 0, tiles = 0;
+        uint64_t prev_end = meta_p, ts = 0, tl = 0, tiles = 0, tiles_s = 0;
         for (uint64_t b = 0; b < nb && rc == ACEAPEX_OK; ++b) {
             const uint64_t po = rd64(dir + 16 * b); const uint32_t ns = rd32(dir + 16 * b + 8), nl = rd32(dir + 16 * b + 12);
             if ((po & 127) || po < prev_end || ns == 0) { rc = ACEAPEX_E_HEADER; break; }
             const uint64_t bytes = 3 * pad16(2ull * ns) + pad16(4ull * ns) + pad16(nl);
             if (po > comp_bytes || bytes > comp_bytes - po) { rc = ACEAPEX_E_TRUNCATED; break; }
-            prev_end = po + bytes; ts += ns; tl += nl; tiles += (ns + TILE - 1) / TILE;
+            prev_end = po + bytes; ts += ns; tl += nl; tiles += (ns + TILE_LIST - 1) / TILE_LIST; tiles_s += (ns + TILE_STREAM - 1) / TILE_STREAM;
         }
         if (rc) break;
-        if (ts != p->total_seq || tl != p->total_lit || tl > p->raw_size || tiles > 0xFFFFFFF0ull) { rc = ACEAPEX_E_HEADER; break; }
-        p->n_tiles = (uint32_t)tiles;
+        if (ts != p->total_seq || tl != p->total_lit || tl > p->raw_size || tiles_s > 0xFFFFFFF0ull) { rc = ACEAPEX_E_HEADER; break; }
+        p->n_tiles_list = (uint32_t)tiles; p->n_tiles_stream = (uint32_t)tiles_s;
         p->hist_cnt.resize(p->max_depth + 1); p->hist_bytes.resize(p->max_depth + 1);
         uint64_t nm = 0, mb = 0;
         for (uint32_t d = 0; d <= p->max_depth; ++d) {
@@ -147,13 +152,13 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         if (ce == cudaSuccess) ce = cudaGetDeviceProperties(&prop, device);
         if (ce == cudaSuccess) ce = pre_configure();
         if (ce == cudaSuccess) ce = waves_configure();
-        if (ce == cudaSuccess) ce = span_configure();
+        if (ce == cudaSuccess) ce = chain_configure();
         if (ce == cudaSuccess) ce = pass_configure();
         if (ce != cudaSuccess) { p->last_cuda = (int)ce; rc = ACEAPEX_E_CUDA; cudaGetLastError(); break; }
         p->device = device; p->n_sm = prop.multiProcessorCount;
         int pre_occ = pre_max_ctas_per_sm(p->max_depth); if (pre_occ < 1) pre_occ = 1;
         p->pre_grid = p->n_sm * pre_occ;
-        { int so = span_max_ctas_per_sm(); if (so < 1) so = 1; p->span_grid = p->n_sm * so; }
+        { int so = chain_max_ctas_per_sm(); if (so < 1) so = 1; p->chain_grid = p->n_sm * so; }
         { int po = pass_max_ctas_per_sm(); if (po < 1) po = 1; p->pass_grid = p->n_sm * po; }
         p->match_ctas_per_sm = match_max_ctas_per_sm(); if (p->match_ctas_per_sm < 1) p->match_ctas_per_sm = 1;
         if (cur >= 0 && cur != device) cudaSetDevice(cur);
@@ -163,8 +168,8 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_wave_off = o; o += up256(4ull * (p->max_depth + 2));
         p->o_cursor = o; o += up256(4ull * (p->max_depth + 2));
         p->o_blocks = o; o += up256(sizeof(BlockDesc) * (size_t)nb);
-        p->o_tiles = o; o += up256(8ull * p->n_tiles);
-        p->o_tblk = o; o += up256(4ull * p->n_tiles);
+        p->o_tiles = o; o += up256(8ull * p->n_tiles_stream);       // (sized for the finer tiling)
+        p->o_tblk = o; o += up256(4ull * p->n_tiles_stream);
         p->o_chain = o; o += up256(4ull * chain_sync_words((uint32_t)nb));
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
@@ -185,9 +190,8 @@ extern "C" size_t aceapex_scratch_bytes(const aceapex_plan_t* p) { return p ? p-
 extern "C" int aceapex_last_cuda_error(const aceapex_plan_t* p) { return p ? p->last_cuda : 0; }
 
 extern "C" int aceapex_set_strategy(aceapex_plan_t* p, int s) {
-    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_PASSES) return ACEAPEX_E_ARG;
+    if (!p || s < ACEAPEX_WAVES_AUTO || s > ACEAPEX_WAVES_CHAIN) return ACEAPEX_E_ARG;
     if (s == ACEAPEX_WAVES_PASSES && p->max_depth > PASS_MAX_DEPTH) return ACEAPEX_E_ARG;
-    if (s == ACEAPEX_WAVES_SPAN && p->max_depth == 0) return ACEAPEX_E_ARG;
     if (s == ACEAPEX_WAVES_CHAIN && !(p->flags & FLAG_FLATTENED)) return ACEAPEX_E_ARG;   // needs invariant I3
     p->strategy_forced = s;
     return ACEAPEX_OK;
@@ -208,10 +212,10 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
     P.raw_size = p->raw_size; P.comp_bytes = p->comp_bytes; P.block_size = p->block_size; P.n_blocks = p->n_blocks;
-    P.n_tiles = p->n_tiles; P.max_depth = p->max_depth; P.min_match = p->min_match;
-    // strategy SPAN: the last depth has no wave list (k_span copies it straight from the stream)
-    // strategy CHAIN: no wave list at all (k_span<true> copies every match straight from the stream, in block order)
-    P.list_hi = strategy == ACEAPEX_WAVES_CHAIN ? 0 : strategy == ACEAPEX_WAVES_SPAN ? p->max_depth - 1 : p->max_depth;
+    const bool stream_tiles = strategy == ACEAPEX_WAVES_PASSES || strategy == ACEAPEX_WAVES_CHAIN;
+    P.tile = stream_tiles ? TILE_STREAM : TILE_LIST; P.n_tiles = stream_tiles ? p->n_tiles_stream : p->n_tiles_list; P.max_depth = p->max_depth; P.min_match = p->min_match;
+    // strategy CHAIN: no wave list at all (k_chain copies every match straight from the stream, in block order)
+    P.list_hi = strategy == ACEAPEX_WAVES_CHAIN ? 0 : p->max_depth;
     uint64_t nl = 0;
     for (uint32_t d = 1; d <= P.list_hi; ++d) nl += p->hist_cnt[d];
     P.n_list = (uint32_t)nl;
@@ -223,7 +227,7 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
     uint32_t n = 0;
     *n_launch = 0;
     if (p->n_blocks == 0) return cudaSuccess;
-    const bool span = strategy == ACEAPEX_WAVES_SPAN, chain = strategy == ACEAPEX_WAVES_CHAIN;
+    const bool chain = strategy == ACEAPEX_WAVES_CHAIN;
     if (strategy == ACEAPEX_WAVES_PASSES) {
         if (phases & ACEAPEX_PHASE_PRE) {
             // short matches are OR-merged into the output (copy.cuh merge16): start from zeros
@@ -232,12 +236,12 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
                 if (ez != cudaSuccess) return ez;
             }
             launch_index(P, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
-            n += 2 + (p->n_tiles ? 1 : 0);
+            n += 2 + (P.n_tiles ? 1 : 0);
         }
         if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
             // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
             launch_pass_reset(P, st); ++n;
-            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); n += p->n_tiles ? 1 : 0; }
+            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); n += P.n_tiles ? 1 : 0; }
             launch_check_cursors(P, st); ++n;
         }
         *n_launch = n;
@@ -251,19 +255,20 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
         }
         launch_index(P, st); ++n;
         launch_tilesum(P, p->n_sm * 8, st); ++n;
-        launch_pre(P, p->pre_grid, st); n += (p->n_tiles ? 1 : 0) + (P.list_hi ? 1 : 0);
+        if (chain) { launch_pass(P, 0, p->pass_grid, st); n += P.n_tiles ? 1 : 0; }   // literal scatter only: the chain pass validates and counts
+        else { launch_pre(P, p->pre_grid, st); n += (P.n_tiles ? 1 : 0) + (P.list_hi ? 1 : 0); }
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
     if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth && chain) {
-        // one pass over the token stream in block order (replayable: counts and frontier restart from zero)
-        cudaError_t e = cudaMemsetAsync(&P.status->n_final, 0, sizeof(uint32_t), st);
-        if (e == cudaSuccess) e = launch_chain(P, p->span_grid, st);
+        // one pass over the token stream in block order (replayable: counts, M_src and frontier restart from zero)
+        cudaError_t e = cudaMemsetAsync(&P.status->match_src_bytes, 0, sizeof(unsigned long long) + sizeof(uint32_t), st);
+        if (e == cudaSuccess) e = launch_chain(P, p->chain_grid, st);
         if (e != cudaSuccess) return e;
-        n += p->n_tiles ? 1 : 0;
+        n += P.n_tiles ? 1 : 0;
     } else if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
         const int wave_grid = p->n_sm * p->match_ctas_per_sm;
-        if (strategy == ACEAPEX_WAVES_PERSISTENT || (span && P.list_hi > 8)) {
+        if (strategy == ACEAPEX_WAVES_PERSISTENT) {
             cudaError_t e = launch_waves_persistent(P, 1, P.list_hi, wave_grid, st);
             if (e != cudaSuccess) return e;
             ++n;
@@ -273,12 +278,6 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
                 if (e != cudaSuccess) return e;
                 if (p->hist_cnt[d]) ++n;
             }
-        }
-        if (span) {
-            // the last depth: one streaming pass writes the whole output (replayable: the count starts from zero)
-            cudaError_t e = cudaMemsetAsync(&P.status->n_final, 0, sizeof(uint32_t), st);
-            if (e != cudaSuccess) return e;
-            launch_span(P, p->max_depth, p->span_grid, st); n += p->n_tiles ? 1 : 0;
         }
     }
     *n_launch = n;
@@ -378,9 +377,8 @@ extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, ace
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
         s->match_src_bytes = h.match_src_bytes; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
         // strategy SPAN keeps no list (hence no cursor) for the last depth: its count comes back from the span pass
-        const uint64_t want_final = p->last_strategy == ACEAPEX_WAVES_SPAN ? p->hist_cnt[p->max_depth] : p->n_match;
-        if (!h.fault_flags && (p->last_strategy == ACEAPEX_WAVES_SPAN || p->last_strategy == ACEAPEX_WAVES_CHAIN) && p->max_depth &&
-            p->last_had_match && h.n_final != want_final) {
+        // strategy CHAIN keeps no list (hence no cursor): its match count comes back from the chain pass
+        if (!h.fault_flags && p->last_strategy == ACEAPEX_WAVES_CHAIN && p->max_depth && p->last_had_match && h.n_final != p->n_match) {
             s->fault_flags = F_DEPTH; s->fault_block = 0xFFFFFFFEu;
         }
         if (s->fault_flags) return ACEAPEX_E_STREAM;

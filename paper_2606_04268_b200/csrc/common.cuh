@@ -13,10 +13,15 @@ constexpr uint32_t FLAG_FLATTENED = 1, FLAG_DEPTH_LIMITED = 2, FLAG_HAS_DEP = 4;
 // ---- fault bits (include/aceapex.h ACEAPEX_F_*)
 constexpr uint32_t F_BLOCK_SUM = 1, F_SOURCE = 2, F_DEPTH = 4, F_PLACEHOLDER = 8, F_INDEX = 16;
 
-// ---- tiling of the token stream: one tile = TILE consecutive sequences of one block
-constexpr int PRE_THREADS = 256;
+// ---- tiling of the token stream: one tile = Params::tile consecutive sequences of one block.  The tile size belongs to
+// the strategy: the bucketing kernel (k_pre: wave lists) sorts a tile's matches in shared memory and likes them large;
+// the streaming kernels (k_pass, k_chain) want many small CTAs — measured on text1g_d4: PASSES 5.15 ms at 2048, 4.86 ms
+// at 512; on fastq1g: k_pre 2.4 ms at 2048, 3.5 ms at 512; CHAIN 8.95 ms at 2048, 7.8 ms at 512.
 constexpr int PRE_ITEMS = 8;                       // consecutive sequences per thread (8 x u16 = one 16 B load)
-constexpr int TILE = PRE_THREADS * PRE_ITEMS;      // 2048
+constexpr int PRE_THREADS = 256;                   // k_pre
+constexpr int TILE_LIST = PRE_THREADS * PRE_ITEMS; // 2048: strategies LAUNCH / GRAPH / PERSISTENT
+constexpr int PS_THREADS = 64;                     // k_pass
+constexpr int TILE_STREAM = PS_THREADS * PRE_ITEMS;// 512: strategies PASSES / CHAIN
 constexpr uint32_t PASS_MAX_DEPTH = 16;               // strategy PASSES: one streaming pass per depth, at most this many
 constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in shared memory; deeper streams use global atomics
 
@@ -39,7 +44,7 @@ struct Status {
     uint32_t fault_flags;
     uint32_t fault_block;                          // atomicMin; 0xFFFFFFFF = none
     unsigned long long match_src_bytes;            // M_src counted during PRE
-    uint32_t n_final;                              // matches of the last depth copied by the span pass (histogram check)
+    uint32_t n_final;                              // matches copied by the chain pass (checked against the header)
     uint32_t pad0[27];
     uint32_t barrier;                              // grid barrier counter of the persistent wave kernel
     uint32_t pad1[31];
@@ -61,10 +66,9 @@ struct Params {
     uint32_t* wl_off;                              // [n_list] match source (absolute)
     uint16_t* wl_len;                              // [n_list]
     uint64_t raw_size, comp_bytes;
-    uint32_t block_size, n_blocks, n_tiles, max_depth, min_match;
+    uint32_t block_size, n_blocks, n_tiles, tile, max_depth, min_match;   // tile: sequences per tile (TILE_LIST or TILE_STREAM)
     uint32_t n_list;                               // capacity of the wave lists = matches at depths 1 .. list_hi
-    uint32_t list_hi;                              // depths 1 .. list_hi travel through wave lists; deeper ones (strategy
-                                                   // SPAN: the last depth) are copied by the span pass straight from the stream
+    uint32_t list_hi;                              // depths 1 .. list_hi travel through wave lists (0: strategy CHAIN, no lists)
 };
 
 __host__ __device__ inline uint64_t pad16(uint64_t x) { return (x + 15) & ~(uint64_t)15; }
@@ -91,10 +95,8 @@ __device__ __forceinline__ void parse8(Seq8& s, uint4 vc, uint4 vl, uint4 vd, ui
     for (int k = 0; k < PRE_ITEMS; ++k) if ((uint32_t)k >= n_valid) { s.c[k] = 0; s.l[k] = 0; s.dp[k] = 0; s.of[k] = 0; }
 }
 
-// The same from global memory: sequences j0 .. j0+7 of block B (j0 a multiple of 8).  need_src = false skips dep[] / off[];
-// sel_depth != 0 loads off[] (32 of the 80 bytes) only if one of the eight sequences sits at that depth — a pass over a
-// sparse depth then reads 6 instead of 10 bytes for most sequences.
-__device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const BlockDesc& B, uint32_t j0, bool need_src, uint32_t sel_depth = 0) {
+// The same from global memory: sequences j0 .. j0+7 of block B (j0 a multiple of 8).  need_src = false skips dep[] / off[].
+__device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const BlockDesc& B, uint32_t j0, bool need_src) {
     const uint4 z = make_uint4(0u, 0u, 0u, 0u);
     if (j0 >= B.n_seq) { parse8(s, z, z, z, z, z, 0); return; }
     const uint4 vc = *reinterpret_cast<const uint4*>(comp + B.cmd_off + 2ull * j0);
@@ -102,17 +104,8 @@ __device__ __forceinline__ void load_seq8(Seq8& s, const uint8_t* comp, const Bl
     uint4 vd = z, o0 = z, o1 = z;
     if (need_src) {
         vd = *reinterpret_cast<const uint4*>(comp + B.dep_off + 2ull * j0);
-        bool want = true;
-        if (sel_depth) {
-            const uint32_t lo = sel_depth | (sel_depth << 16);                 // any 16-bit lane of vd equal to sel_depth?
-            const uint32_t x0 = vd.x ^ lo, x1 = vd.y ^ lo, x2 = vd.z ^ lo, x3 = vd.w ^ lo;
-            auto has_zero16 = [](uint32_t x) { return ((x & 0xFFFFu) == 0u) || ((x >> 16) == 0u); };
-            want = has_zero16(x0) || has_zero16(x1) || has_zero16(x2) || has_zero16(x3);
-        }
-        if (want) {
-            o0 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0);
-            o1 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0 + 16);
-        }
+        o0 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0);
+        o1 = *reinterpret_cast<const uint4*>(comp + B.off_off + 4ull * j0 + 16);
     }
     parse8(s, vc, vl, vd, o0, o1, B.n_seq - j0);
 }

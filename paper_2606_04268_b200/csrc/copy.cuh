@@ -48,6 +48,41 @@ __device__ __forceinline__ void store16(uint8_t* q, V16 v, uint32_t n) {
     if (n & 1) *q = (uint8_t)v.lo;
 }
 
+// The same contract as store16 (exactly the bytes [q, q+n), n in 1..16, naturally aligned 1/2/4-byte stores), built for
+// latency instead of store count: the value is shifted once to the destination's phase inside its 4-byte word (five
+// words, independent funnel shifts) and every possible piece — up to three head bytes, four whole words, up to three
+// tail bytes — is a predicated store of one of them, so nothing waits on the previous piece (store16's pieces are a
+// chain of shifts).  Used for the shared-memory image of the tile pass, where a warp's stores are its critical path.
+__device__ __forceinline__ void place16(uint8_t* q, V16 v, uint32_t n) {
+    const uint32_t a = (uint32_t)(uintptr_t)q & 3u, sh = a * 8u, e = a + n;           // e: end byte (exclusive) relative to word 0
+    uint8_t* const q0 = q - a;
+    const uint32_t s0 = (uint32_t)v.lo, s1 = (uint32_t)(v.lo >> 32), s2 = (uint32_t)v.hi, s3 = (uint32_t)(v.hi >> 32);
+    const uint32_t w0 = s0 << sh, w1 = __funnelshift_l(s0, s1, sh), w2 = __funnelshift_l(s1, s2, sh),
+                   w3 = __funnelshift_l(s2, s3, sh), w4 = __funnelshift_l(s3, 0u, sh);
+    // word 0: bytes [a, min(4, e))
+    const uint32_t h = e < 4u ? e : 4u;
+    if (a == 0u && h == 4u) *reinterpret_cast<uint32_t*>(q0) = w0;
+    else {
+        uint32_t p = a;
+        if ((p & 1u) && p < h) { q0[p] = (uint8_t)(w0 >> (8u * p)); ++p; }
+        if (p + 2u <= h) { *reinterpret_cast<uint16_t*>(q0 + p) = (uint16_t)(w0 >> (8u * p)); p += 2u; }
+        if (p < h) q0[p] = (uint8_t)(w0 >> (8u * p));
+    }
+    // whole words 1 .. 4
+    if (e >= 8u) *reinterpret_cast<uint32_t*>(q0 + 4) = w1;
+    if (e >= 12u) *reinterpret_cast<uint32_t*>(q0 + 8) = w2;
+    if (e >= 16u) *reinterpret_cast<uint32_t*>(q0 + 12) = w3;
+    if (e >= 20u) *reinterpret_cast<uint32_t*>(q0 + 16) = w4;     // (n = 16, a = ... never: e <= 19; kept for completeness)
+    // tail: bytes [4k, e) of word k = e / 4 >= 1
+    const uint32_t k = e >> 2, t = e & 3u;
+    if (k >= 1u && t) {
+        const uint32_t wk = k == 1u ? w1 : k == 2u ? w2 : k == 3u ? w3 : w4;
+        uint8_t* const qk = q0 + 4u * k;
+        if (t & 2u) *reinterpret_cast<uint16_t*>(qk) = (uint16_t)wk;
+        if (t & 1u) qk[t & 2u] = (uint8_t)(wk >> (8u * (t & 2u)));
+    }
+}
+
 // OR-merge the first n (1..16) bytes of v into ZEROED memory at q with 8-byte reductions (red.global.or.b64): one L2
 // operation per aligned word touched (1 + (n-1)/8 on average) instead of one per naturally aligned piece (~3 for a
 // 9-byte match).  Measured on B200: the L2 sustains scattered sub-word writes at a rate set by their COUNT

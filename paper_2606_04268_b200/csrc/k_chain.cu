@@ -1,59 +1,54 @@
-// k_span.cu — the tile pass: one streaming pass over the token stream that writes every output byte of its matches
-// exactly once, coalesced, with no wave list, no atomics on the output and no zeroed output.  Two uses:
-//   strategy SPAN  (CHAIN = false)  the LAST match wave of a shallow stream (the depth-limited encoder of PAPER.md:228 §7.4
-//       piles most matches up at depth D): depths 1 .. D-1 went through wave lists, this pass copies depth D.
-//   strategy CHAIN (CHAIN = true)   EVERY match of a FLATTENED stream: after chain flattening no match reads bytes
-//       produced by another match of its own block (§3.3, invariant I3), so once the literal scatter has
-//       run, every match of block b depends on blocks < b only.  Tiles are taken in file order; a tile that holds a
-//       match of depth > 1 with a source before its block waits for the FRONTIER (number of leading blocks completely
-//       written) to reach its block; the tile that completes block b publishes frontier = b + 1.  One flag hop per 1 MB
-//       block replaces one grid barrier per depth ("synchronization-bound"); dep[] is used only to skip
-//       the wait (dep == 1: all sources are literals).
-// Per tile (2048 sequences of one block, 512 threads, 2 CTAs per SM):
+// k_chain.cu — strategy CHAIN: every match of a FLATTENED stream in ONE streaming pass over the token stream that writes
+// every output byte exactly once, coalesced, with no wave list, no atomics on the output and no zeroed output.
+// After chain flattening no match reads bytes produced by another match of its own block (§3.3, invariant
+// I3), so once the literal scatter has run, every match of block b depends on blocks < b only.  Tiles are taken in file
+// order; a tile that holds a match of depth > 1 with a source before its block waits until every earlier block is
+// completely written (a7: per-block completion counts + a frontier word instead of one grid barrier per depth —
+// PAPER.md:224 "synchronization-bound"); dep[] is used only to skip the wait (dep == 1: all sources are literals).
+// Per tile (512 sequences of one block, 256 threads, 4 CTAs per SM):
 //   a2  the tile's cmd[] / len[] / dep[] / off[] slices and its slice of lit[] arrive in shared memory by 1-D bulk TMA
-//       (cp.async.bulk + mbarrier); the next tile's descriptor is fetched by one thread while this tile is processed
-//   a3  scan inside the tile: each thread sums 4 CONSECUTIVE sequences, warp shuffles + one barrier give every token's
+//       (cp.async.bulk + mbarrier); the next tile's descriptor is fetched by one thread (cp.async) meanwhile
+//   a3  scan inside the tile: each thread sums 2 CONSECUTIVE sequences, warp shuffles + one barrier give every token's
 //       output position and literal offset (the tile's prefix inside its block comes from k_tilesum), kept in shared memory
-//   a6  then thread t takes tokens t, t+512, ... (neighbouring lanes = neighbouring tokens: neighbouring sources share
-//       L1 lines, neighbouring destinations share image words):
-//         gather   the aligned 8-byte words holding each short match's source travel global -> shared with cp.async
-//                  (no registers held across the round trip; all of a thread's tokens in flight at once)
-//         assemble every token is written into a shared-memory IMAGE of the tile's output span with naturally aligned
-//                  1/2/4/8-byte stores (each byte has one owner: no merge, no zero fill):
-//                    literal run          <- lit[]
-//                    match being copied   <- out[off ..), periodic if it overlaps   (Q3)
-//                    other matches (SPAN) <- out[mdst ..) (their own bytes, already written by their wave)
-//                  tokens longer than 16 bytes are copied by the whole warp
+//   a6  then thread t takes tokens t, t+256 (neighbouring lanes = neighbouring tokens: neighbouring sources share L1
+//       lines, neighbouring destinations share image words):
+//         before the wait  literal runs go into a shared-memory IMAGE of the tile's output span; each match is reduced to
+//                          (aligned source address, destination, length / phase / period)
+//         gather           the aligned 8-byte words holding each match's source travel global -> shared with cp.async
+//                          (no registers held across the round trip; all of a thread's tokens in flight at once)
+//         assemble         every match is written into the image with naturally aligned 1/2/4-byte stores (each byte has
+//                          one owner: no merge, no zero fill), periodic if it overlaps its source (Q3); matches
+//                          up to 32 bytes by one thread, longer ones by the whole warp
 //       and the image goes to global memory with one bulk TMA store (16-byte chunks; <= 15 head / tail bytes by byte
 //       stores).  Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight
-//       to global memory instead.
-// Rewriting a byte with its own value while another CTA reads it as a match source is harmless: a reader sees the old
-// or the new copy of the same value.
+//       to global memory instead (their literal runs are there already: the literal scatter ran before).
+// Rewriting a literal byte with its own value while another CTA reads it as a match source is harmless: a reader sees the
+// old or the new copy of the same value.
 #include "common.cuh"
 #include "copy.cuh"
 
 namespace ax {
 
-constexpr int SP_PER = 4;                            // tokens per thread
-constexpr int SP_THREADS = TILE / SP_PER;            // 512
+constexpr int TILE = TILE_STREAM;                    // 512 sequences per tile
+constexpr int SP_PER = 2;                            // tokens per thread (measured: 4 -> 2 cuts the hop from 10.3 to 8.1 us at 2048,
+                                                     // and a 512-sequence tile spreads a block's ~370 tiles over all SMs: 7.1 us)
+constexpr int SP_THREADS = TILE / SP_PER;            // 256
 constexpr int SP_WARPS = SP_THREADS / 32;
-constexpr int SP_OCC = 4096 / TILE;                  // CTAs per SM the shared-memory layout below is sized for (2 at TILE = 2048)
+constexpr int SP_OCC = 4;                            // CTAs per SM: 592 resident tiles = 1.6 blocks of a stream of 5.6-byte matches
 constexpr uint32_t SP_STRM = TILE * 10u;             // cmd | len | dep (2 B each) | off (4 B) per sequence
 constexpr uint32_t SP_O_LEN = TILE * 2u, SP_O_DEP = TILE * 4u, SP_O_OFF = TILE * 6u;
-#ifndef AX_SP_IMG
-#define AX_SP_IMG (10 * TILE)
-#endif
-constexpr uint32_t SP_IMG = AX_SP_IMG;               // image capacity in bytes (a text / FASTQ tile of 2048 sequences spans ~12 KB)
-constexpr uint32_t SP_LIT = 2 * TILE;                // staged slice of the block's lit[] (a text tile holds ~400 literal bytes)
-constexpr uint32_t SP_SHORT = 16;                    // tokens up to this length are copied by one thread
-static_assert(SP_THREADS % 32 == 0 && SP_THREADS * SP_PER == TILE, "one tile per CTA step, 4 sequences per thread");
+constexpr uint32_t SP_IMG = 10 * TILE;               // image capacity in bytes (a text / FASTQ tile of 512 sequences spans ~3 KB)
+constexpr uint32_t SP_LIT = 2 * TILE;                // staged slice of the block's lit[] (a text tile holds ~100 literal bytes)
+constexpr uint32_t SP_SHORT = 16;                    // literal runs and self-overlapping matches up to this length: one thread
+constexpr uint32_t SP_SHORT2 = 32;                   // other matches up to this length: one thread, two 16-byte pieces
+static_assert(SP_THREADS % 32 == 0 && SP_THREADS <= 1024 && SP_THREADS * SP_PER == TILE, "one tile per CTA step");
 
 // What one tile needs, gathered by the thread that issues its loads (while the previous tile is processed), so that the
 // CTA does not walk tile_blk[] -> blocks[] -> tile_state[] (dependent global loads) on its critical path.
 struct TileMeta {
     unsigned long long pre;                          // (out << 32 | lit) prefix of the tile inside its block
     const uint8_t* lit;                              // the block's lit[] in global memory
-    uint32_t b, blk_lo, nt, blk_tiles;               // block, its first output byte, sequences in the tile, tiles in the block
+    uint32_t b, blk_lo, nt, blk_tiles, prev_tiles;   // block, its first output byte, sequences in the tile, tiles of blocks b and b-1
     uint32_t lit16, lit_ok;                          // slit[0] = lit[lit16]; lit_ok: the tile's literal bytes are staged
 };
 
@@ -63,7 +58,7 @@ struct TileMeta {
 struct alignas(16) TileFetch {
     BlockDesc B;                                     // 64 bytes, 16-byte aligned in scratch
     unsigned long long pre, pre1;                    // tile_state[tile], tile_state[tile + 1]
-    uint32_t b, pad[3];
+    uint32_t b, prev_tiles, pad[2];                  // prev_tiles: tiles of block b-1 (0 for b = 0)
 };
 static_assert(sizeof(BlockDesc) == 64, "BlockDesc travels as four 16-byte cp.async");
 
@@ -72,7 +67,7 @@ struct SpanSmem {
     alignas(128) uint8_t slit[SP_LIT + 32];
     alignas(16) uint32_t pos[TILE];                  // absolute output position of token j's literal run; later its source address
     alignas(16) uint32_t lpos[TILE];                 // offset of token j's literal run inside the block's lit[]; later its copy info
-    alignas(16) unsigned long long x0[TILE], x1[TILE], x2[TILE];   // the aligned words holding token j's source bytes
+    alignas(16) unsigned long long x0[TILE], x1[TILE], x2[TILE], x3[TILE], x4[TILE];   // the aligned words holding token j's source bytes
     alignas(128) uint8_t img[SP_IMG + 64];
     alignas(8) unsigned long long mbar;
     TileFetch fetch;                                 // (thread 0) descriptor of the next tile
@@ -130,6 +125,8 @@ __device__ __forceinline__ void fetch_step2(const Params& P, TileFetch& F) {
     uint8_t* dst = reinterpret_cast<uint8_t*>(&F.B);
 #pragma unroll
     for (int i = 0; i < 4; ++i) cp_async16(dst + 16 * i, src + 16 * i);
+    if (F.b) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(&F.prev_tiles)), "l"(&P.blocks[F.b - 1].n_seq) : "memory");
+    else F.prev_tiles = 0;                           // (holds n_seq of block b-1 until issue_tile_loads turns it into a tile count)
     asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
@@ -145,7 +142,7 @@ __device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, u
     const bool lit_ok = lbytes <= SP_LIT;
     TileMeta& M = S.meta;
     M.pre = F.pre; M.lit = P.comp + F.B.lit_off; M.b = F.b; M.blk_lo = (uint32_t)F.B.out_base; M.nt = n;
-    M.blk_tiles = (F.B.n_seq + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
+    M.blk_tiles = (F.B.n_seq + TILE - 1) / TILE; M.prev_tiles = (F.prev_tiles + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
     const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
     mbar_expect_tx(&S.mbar, 3 * b2 + b4 + (lit_ok ? lbytes : 0u));
     bulk_load(S.strm, P.comp + F.B.cmd_off + 2ull * j0, b2, &S.mbar);
@@ -174,11 +171,11 @@ __device__ __forceinline__ V16 extract16(unsigned long long x0, unsigned long lo
     return v;
 }
 
-// chain_sync[0] = frontier (blocks 0 .. frontier-1 are completely written); chain_sync[32 + b] = finished tiles of block b
+// chain_sync[0] = frontier word (blocks 0 .. frontier-1 are completely written; trails the truth by up to one hop);
+// chain_sync[32 + b] = finished tiles of block b (block b is complete when it reaches the block's tile count)
 constexpr uint32_t CH_CNT0 = 32;
 
-template <bool CHAIN>
-__global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t depth_hi) {
+__global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SpanSmem& S = *reinterpret_cast<SpanSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
@@ -196,6 +193,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
     }
     __syncthreads();
     uint32_t n_copied = 0;
+    unsigned long long src_bytes = 0;                // M_src (this pass is the one that validates every match)
     uint16_t* const s_cmd = reinterpret_cast<uint16_t*>(S.strm);
     uint16_t* const s_len = reinterpret_cast<uint16_t*>(S.strm + SP_O_LEN);
     uint16_t* const s_dep = reinterpret_cast<uint16_t*>(S.strm + SP_O_DEP);
@@ -209,31 +207,24 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
         mbar_wait(&S.mbar, it & 1u);
         const unsigned long long pre = S.meta.pre;
         const uint8_t* const lit = S.meta.lit;
-        const uint32_t b = S.meta.b, blk_lo = S.meta.blk_lo, nt = S.meta.nt, blk_tiles = S.meta.blk_tiles;
+        const uint32_t b = S.meta.b, blk_lo = S.meta.blk_lo, nt = S.meta.nt, blk_tiles = S.meta.blk_tiles, prev_tiles = S.meta.prev_tiles;
         const uint8_t* const lsrc_base = S.meta.lit_ok ? S.slit - S.meta.lit16 : lit;   // byte x of the block's lit[] is lsrc_base[x]
         const uint32_t A0 = blk_lo + (uint32_t)(pre >> 32);               // absolute start of the tile's span
         const uint32_t img_org = A0 & ~15u;                               // absolute position of image byte 0
         // ================= phase S (thread t owns sequences 4t .. 4t+3): a3 scan, token validation
         const uint32_t jt = tid * SP_PER;
         uint32_t c4[SP_PER], l4[SP_PER], d4[SP_PER], o4[SP_PER];
-        {
-            uint2 vc = make_uint2(0u, 0u), vl = vc, vd = vc; uint4 vo = make_uint4(0u, 0u, 0u, 0u);
-            if (jt < nt) {
-                vc = *reinterpret_cast<const uint2*>(s_cmd + jt); vl = *reinterpret_cast<const uint2*>(s_len + jt);
-                vd = *reinterpret_cast<const uint2*>(s_dep + jt); vo = *reinterpret_cast<const uint4*>(s_off + jt);
-            }
-            c4[0] = vc.x & 0xFFFFu; c4[1] = vc.x >> 16; c4[2] = vc.y & 0xFFFFu; c4[3] = vc.y >> 16;
-            l4[0] = vl.x & 0xFFFFu; l4[1] = vl.x >> 16; l4[2] = vl.y & 0xFFFFu; l4[3] = vl.y >> 16;
-            d4[0] = vd.x & 0xFFFFu; d4[1] = vd.x >> 16; d4[2] = vd.y & 0xFFFFu; d4[3] = vd.y >> 16;
-            o4[0] = vo.x; o4[1] = vo.y; o4[2] = vo.z; o4[3] = vo.w;
-        }
-        unsigned long long tsum = 0;
-        bool wait_src = false;                       // CHAIN: a match deeper than 1 reads an earlier block
 #pragma unroll
         for (int k = 0; k < SP_PER; ++k) {
-            if (jt + k >= nt) { c4[k] = 0; l4[k] = 0; }                   // the tail shares its words with nothing: mask
+            const bool in = jt + k < nt;
+            c4[k] = in ? s_cmd[jt + k] : 0u; l4[k] = in ? s_len[jt + k] : 0u; d4[k] = in ? s_dep[jt + k] : 0u; o4[k] = in ? s_off[jt + k] : 0u;
+        }
+        unsigned long long tsum = 0;
+        bool wait_src = false;                       // a match deeper than 1 reads an earlier block
+#pragma unroll
+        for (int k = 0; k < SP_PER; ++k) {
             tsum += ((unsigned long long)(c4[k] + l4[k]) << 32) | c4[k];
-            if (CHAIN) wait_src |= l4[k] != 0 && o4[k] < blk_lo && d4[k] != 1u;
+            wait_src |= l4[k] != 0 && o4[k] < blk_lo && d4[k] != 1u;
         }
         unsigned long long inc = tsum;
 #pragma unroll
@@ -261,16 +252,14 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
                 const uint32_t mdst = p + c4[k];
                 if (l4[k]) {                                               // token validation (I2, depth range, I3)
                     if (o4[k] >= mdst || l4[k] < P.min_match) bad_src |= 1u << k;
-                    else if (d4[k] == 0 || d4[k] > (CHAIN ? P.max_depth : depth_hi)) bad_dep |= 1u << k;
-                    else if (CHAIN && o4[k] >= blk_lo && d4[k] != 1u) bad_dep |= 1u << k;   // an in-block source that is not literal
+                    else if (d4[k] == 0 || d4[k] > P.max_depth) bad_dep |= 1u << k;
+                    else if (o4[k] >= blk_lo && d4[k] != 1u) bad_dep |= 1u << k;   // an in-block source that is not literal
                 }
                 p = mdst + l4[k]; ls += c4[k];
                 if (p - img_org <= SP_IMG) fit_end = p;                   // tokens are monotone: a prefix of the tile fits the image
             }
-            if (jt < nt) {
-                *reinterpret_cast<uint4*>(S.pos + jt) = make_uint4(ps[0], ps[1], ps[2], ps[3]);
-                *reinterpret_cast<uint4*>(S.lpos + jt) = make_uint4(lp[0], lp[1], lp[2], lp[3]);
-            }
+#pragma unroll
+            for (int k = 0; k < SP_PER; ++k) if (jt + k < nt) { S.pos[jt + k] = ps[k]; S.lpos[jt + k] = lp[k]; }
             if (bad_src | bad_dep) {                                      // a faulty match is flagged and skipped: its bytes stay a hole
 #pragma unroll
                 for (int k = 0; k < SP_PER; ++k) if ((bad_src | bad_dep) & (1u << k)) s_len[jt + k] = 0;
@@ -287,7 +276,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
         // literal runs go into the image, and each match is reduced to what the copy needs —
         //   pos[j]  <- aligned source address (short match) / source address (long match)
         //   lpos[j] <- info: len (16 bits) | source byte phase (3) | period if the source overlaps, else 0 (4) | in image |
-        //              being copied by this pass | valid
+        //              copied by one thread (else by the whole warp)
         //   off[j]  <- match destination
 #pragma unroll 1
         for (uint32_t j0 = warp * 32u; j0 < nt; j0 += SP_THREADS) {
@@ -297,7 +286,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
             const uint32_t ps = live ? S.pos[j] : 0u, lp = live ? S.lpos[j] : 0u;
             const uint32_t pp = ps + c;
             const bool in_img = pp + l - img_org <= SP_IMG;
-            if (c && in_img && c <= SP_SHORT) store16(S.img + (ps - img_org), load16(lsrc_base + lp, c), c);
+            if (c && in_img && c <= SP_SHORT) place16(S.img + (ps - img_org), load16(lsrc_base + lp, c), c);
             uint32_t m = __ballot_sync(0xFFFFFFFFu, c > SP_SHORT && in_img);
             while (m) {                                                   // long literal runs: the whole warp copies each
                 const int sl = __ffs(m) - 1; m &= m - 1;
@@ -307,28 +296,31 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
             if (live) {
                 uint32_t inf = 0, sa = 0;
                 if (l) {
-                    const bool deep = CHAIN || s_dep[j] == depth_hi;
-                    if (in_img || deep) {
-                        const uint32_t of = s_off[j];
-                        const uint32_t src = deep ? of : pp, dist = pp - of;
-                        const bool ovl = deep && dist < l && l <= SP_SHORT;
-                        sa = l <= SP_SHORT ? (src & ~7u) : src;
-                        inf = l | (src & 7u) << 16 | (ovl ? dist : 0u) << 19 | (in_img ? 1u << 23 : 0u) | (deep ? 1u << 24 : 0u) | 1u << 25;
-                        if (deep) ++n_copied;
-                    }
+                    const uint32_t of = s_off[j], dist = pp - of;
+                    const bool ovl = dist < l;
+                    const bool by_thread = l <= SP_SHORT || (l <= SP_SHORT2 && !ovl);
+                    sa = by_thread ? (of & ~7u) : of;
+                    inf = l | (of & 7u) << 16 | (ovl && by_thread ? dist : 0u) << 19 | (in_img ? 1u << 23 : 0u) | (by_thread ? 1u << 26 : 0u);
+                    ++n_copied; src_bytes += ovl ? dist : l;
                 }
                 S.pos[j] = sa; S.lpos[j] = inf; s_off[j] = pp;
             }
         }
-        if (CHAIN && must_wait) {
-            // a7 for strategy CHAIN: every block before this one completely written?  One thread spins on the frontier;
+        if (must_wait) {
+            // a7: every block before this one completely written?  One thread spins on the frontier;
             // its acquire fence also drops this SM's L1 (CCTL.IVALL), so the loads below see what other SMs wrote.
             if (tid == 0) {
+                // blocks 0 .. b-2: the frontier word (moved by the last tile of every block, in block order, one hop ago);
+                // block b-1: its completion count itself, so that the returning atomic and the frontier store of its last
+                // tile are off the critical path
                 uint32_t v;
                 for (;;) {
                     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory");
-                    if (v >= b) break;
-                    if (v + 1u < b) __nanosleep(400);                     // not next in line: keep the hot line's queue short
+                    if (v + 1u >= b) break;
+                    __nanosleep(400);                                     // not next in line: keep the hot lines' queues short
+                }
+                if (v < b) {
+                    do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory"); } while (v < prev_tiles);
                 }
                 asm volatile("fence.acq_rel.gpu;" ::: "memory");
             }
@@ -340,31 +332,41 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
             const uint32_t j = k * SP_THREADS + tid;
             if (j >= nt) continue;
             const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
-            if (l == 0 || l > SP_SHORT) continue;
+            if (!((inf >> 26) & 1u)) continue;
             const uint32_t per = (inf >> 19) & 15u;
             const uint32_t span = ((inf >> 16) & 7u) + (per ? per : l);
             const uint8_t* g = P.out + S.pos[j];
             cp_async8(&S.x0[j], g);
             if (span > 8u) cp_async8(&S.x1[j], g + 8);
             if (span > 16u) cp_async8(&S.x2[j], g + 16);
+            if (span > 24u) cp_async8(&S.x3[j], g + 24);
+            if (span > 32u) cp_async8(&S.x4[j], g + 32);
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         if (tid == 0 && has_next) prefetch_tile_l2(P, next, F);
         // ================= phase M: a6, every match into the image (or, beyond its capacity, straight to global memory).
-        // The thread's four tokens are unrolled so that their dependent shift / store chains interleave.
+        // The thread's tokens are unrolled so that their dependent shift / store chains interleave.
         bool any_long = false;
 #pragma unroll
         for (int k = 0; k < SP_PER; ++k) {
             const uint32_t j = k * SP_THREADS + tid;
             if (j >= nt) continue;
             const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
-            any_long |= l > SP_SHORT;
-            if (l != 0 && l <= SP_SHORT) {
-                const uint32_t pp = s_off[j], per = (inf >> 19) & 15u;
-                V16 v = extract16(S.x0[j], S.x1[j], S.x2[j], (inf >> 16) & 7u);
+            any_long |= l != 0 && !((inf >> 26) & 1u);
+            if ((inf >> 26) & 1u) {
+                const uint32_t pp = s_off[j], per = (inf >> 19) & 15u, sb = (inf >> 16) & 7u;
+                const unsigned long long y2 = S.x2[j];
+                V16 v = extract16(S.x0[j], S.x1[j], y2, sb);
                 if (per) v = extend_period(v, per);                        // self-overlap: periodic extension (Q3)
-                store16((inf >> 23) & 1u ? S.img + (pp - img_org) : P.out + pp, v, l);
+                const uint32_t l0 = l < 16u ? l : 16u;
+                if ((inf >> 23) & 1u) {
+                    place16(S.img + (pp - img_org), v, l0);
+                    if (l > 16u) place16(S.img + (pp - img_org) + 16, extract16(y2, S.x3[j], S.x4[j], sb), l - 16u);
+                } else {
+                    store16(P.out + pp, v, l0);
+                    if (l > 16u) store16(P.out + pp + 16, extract16(y2, S.x3[j], S.x4[j], sb), l - 16u);
+                }
             }
         }
         if (__any_sync(0xFFFFFFFFu, any_long)) {                          // long matches: the whole warp copies each
@@ -374,15 +376,14 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
                 const bool live = j < nt;
                 const uint32_t inf = live ? S.lpos[j] : 0u, l = inf & 0xFFFFu;
                 const uint32_t pp = live ? s_off[j] : 0u, sa = live ? S.pos[j] : 0u;
-                uint32_t m = __ballot_sync(0xFFFFFFFFu, l > SP_SHORT);
+                uint32_t m = __ballot_sync(0xFFFFFFFFu, l != 0 && !((inf >> 26) & 1u));
                 while (m) {
                     const int sl = __ffs(m) - 1; m &= m - 1;
                     const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, pp, sl), o2 = __shfl_sync(0xFFFFFFFFu, sa, sl),
                                    n2 = __shfl_sync(0xFFFFFFFFu, l, sl), f2 = __shfl_sync(0xFFFFFFFFu, inf, sl);
                     const bool im2 = (f2 >> 23) & 1u;
                     uint8_t* dst = im2 ? S.img + (d2 - img_org) : P.out + d2;
-                    if ((f2 >> 24) & 1u) warp_match(dst, P.out + o2, n2, d2 - o2, !im2, lane);
-                    else warp_copy(dst, P.out + o2, n2, lane);             // (SPAN, image mode only) its own bytes: o2 == d2
+                    warp_match(dst, P.out + o2, n2, d2 - o2, !im2, lane);
                 }
             }
         }
@@ -401,7 +402,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
                 const uint32_t a = c1 + (tid - 16u);
                 if (a < E) P.out[a] = S.img[a - img_org];
             }
-            if (CHAIN) {
+            {
                 // publish: the tile's bytes (bulk store complete, head / tail / direct stores ordered by barrier 4 and the
                 // warp barrier) happen before the release-add; the tile that completes block b moves the frontier, in
                 // block order (blocks whose tiles never had to wait may finish early).
@@ -413,7 +414,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
                 if (tid == 0) {
                     uint32_t old;
                     asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
-                    if (old + 1u == blk_tiles) {
+                    if (old + 1u == blk_tiles) {                          // block b complete: move the frontier word, in block order
                         uint32_t v;
                         do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory"); } while (v < b);
                         asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(P.chain_sync), "r"(b + 1u) : "memory");
@@ -426,39 +427,33 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_span(Params P, uint32_t 
 #pragma unroll
     for (int d = 16; d; d >>= 1) n_copied += __shfl_xor_sync(0xFFFFFFFFu, n_copied, d);
     if (lane == 0 && n_copied) atomicAdd(&P.status->n_final, n_copied);
+    {
+#pragma unroll
+        for (int d = 16; d; d >>= 1) src_bytes += __shfl_xor_sync(0xFFFFFFFFu, src_bytes, d);
+        if (lane == 0 && src_bytes) atomicAdd(&P.status->match_src_bytes, src_bytes);
+    }
 }
 
-size_t span_smem_bytes() { return sizeof(SpanSmem); }
-
-cudaError_t span_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_span<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_span<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
+cudaError_t chain_configure() {
+    return cudaFuncSetAttribute(k_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanSmem));
 }
 
-int span_max_ctas_per_sm() {
-    int n = 0, m = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_span<false>, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m, k_span<true>, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
-    return n < m ? n : m;
+int chain_max_ctas_per_sm() {
+    int n = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain, SP_THREADS, sizeof(SpanSmem)) != cudaSuccess) return 0;
+    return n;
 }
 
-void launch_span(const Params& P, uint32_t depth_hi, int grid, cudaStream_t st) {
-    if (!P.n_tiles) return;
-    const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
-    k_span<false><<<g, SP_THREADS, sizeof(SpanSmem), st>>>(P, depth_hi);
-}
-
-// Strategy CHAIN: every tile of the grid must be resident (a tile spins on the frontier that lower tiles advance), so the
-// launch is cooperative and the grid at most n_sm x occupancy; frontier and per-block counts start from zero.
+// Every tile of the grid must be resident (a tile spins until lower tiles are done), so the launch is cooperative and the
+// grid at most n_sm x occupancy; the frontier word and the per-block counts start from zero.
 cudaError_t launch_chain(const Params& P, int grid, cudaStream_t st) {
     if (!P.n_tiles) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(P.chain_sync, 0, sizeof(uint32_t) * (CH_CNT0 + (size_t)P.n_blocks), st);
     if (e != cudaSuccess) return e;
-    uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles, zero = 0;
+    const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
     Params p = P;
-    void* args[] = {&p, &zero};
-    return cudaLaunchCooperativeKernel((const void*)k_span<true>, dim3(g), dim3(SP_THREADS), args, sizeof(SpanSmem), st);
+    void* args[] = {&p};
+    return cudaLaunchCooperativeKernel((const void*)k_chain, dim3(g), dim3(SP_THREADS), args, sizeof(SpanSmem), st);
 }
 
 size_t chain_sync_words(uint32_t n_blocks) { return CH_CNT0 + (size_t)n_blocks; }

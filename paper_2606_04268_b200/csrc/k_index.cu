@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
     }
     __syncthreads();
     const uint64_t meta = (HDR_BYTES + (uint64_t)DIR_BYTES * P.n_blocks + (uint64_t)HIST_BYTES * (P.max_depth + 1ull) + 127ull) & ~127ull;
-    // ---- block descriptors + tile_base = exclusive prefix of ceil(n_seq / TILE)
+    // ---- block descriptors + tile_base = exclusive prefix of ceil(n_seq / tile)
     uint32_t carry = 0;
     for (uint32_t b0 = 0; b0 < P.n_blocks; b0 += IDX_THREADS) {
         const uint32_t b = b0 + threadIdx.x;
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
             const uint64_t bytes = 3 * pad16(2ull * ns) + pad16(4ull * ns) + pad16(nl);
             ok = !(po & 127) && po >= meta && ns != 0 && po <= P.comp_bytes && bytes <= P.comp_bytes - po;
             if (!ok) { raise_fault(P.status, F_INDEX, b); ns = 0; }
-            nt = (ns + TILE - 1) / TILE;
+            nt = (ns + P.tile - 1) / P.tile;
         }
         uint32_t tot;
         const uint32_t ex = block_excl_scan(nt, s_warp, &tot);

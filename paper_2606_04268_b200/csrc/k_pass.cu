@@ -14,7 +14,7 @@
 
 namespace ax {
 
-constexpr int PS_WARPS = PRE_THREADS / 32;
+constexpr int PS_WARPS = PS_THREADS / 32;
 constexpr int PS_WCAP = 32 * PRE_ITEMS;                  // matches one warp can select in a tile (256)
 
 struct PassSmem {
@@ -27,7 +27,7 @@ struct PassSmem {
 
 // ---- pass p: 0 = literals, p >= 1 = matches of depth p
 template <bool LIT>
-__global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pass(Params P, uint32_t p) {
+__global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P, uint32_t p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PassSmem& S = *reinterpret_cast<PassSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -40,10 +40,10 @@ __global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pass(Params
         const uint32_t b = P.tile_blk[tile];
         const unsigned long long pre = P.tile_state[tile];
         const BlockDesc B = P.blocks[b];
-        const uint32_t j0 = (tile - B.tile_base) * TILE + tid * PRE_ITEMS;
+        const uint32_t j0 = (tile - B.tile_base) * TILE_STREAM + tid * PRE_ITEMS;
         // ---- a2: parse (pass 0 needs neither depths nor sources)
         Seq8 q;
-        load_seq8(q, P.comp, B, j0, !LIT, p == P.max_depth ? 0u : p);     // (the last pass checks every placeholder: it needs every off[])
+        load_seq8(q, P.comp, B, j0, !LIT);
         uint32_t (&c)[PRE_ITEMS] = q.c, (&l)[PRE_ITEMS] = q.l, (&dp)[PRE_ITEMS] = q.dp, (&of)[PRE_ITEMS] = q.of;
         // ---- a3: scan inside the tile; the block-level prefix comes from k_tilesum.  The literal pass scans the pair
         // (cmd+len, cmd) packed in one u64; match passes need output positions only (32-bit shuffles)
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pass(Params
                 const uint32_t mdst = blk_lo + pos;
                 bool sel = ok && l[k] != 0 && dp[k] == p;
                 if (sel && (of[k] >= mdst || l[k] < P.min_match)) { raise_fault(P.status, F_SOURCE, b); sel = false; }   // I2
-                if (p == P.max_depth && l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
+                if (p == 1 && l[k] == 0 && (of[k] | dp[k])) raise_fault(P.status, F_PLACEHOLDER, b);
                 if (sel) { const uint32_t dist = mdst - of[k]; sb += l[k] < dist ? l[k] : dist; }
                 const uint32_t msk = __ballot_sync(0xFFFFFFFFu, sel);
                 if (sel) {
@@ -172,15 +172,15 @@ cudaError_t pass_configure() {
 
 int pass_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PRE_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
     return n;
 }
 
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {
     if (!P.n_tiles) return;
     const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
-    if (p == 0) k_pass<true><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
-    else k_pass<false><<<g, PRE_THREADS, sizeof(PassSmem), st>>>(P, p);
+    if (p == 0) k_pass<true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else k_pass<false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
 }
 
 }  // namespace ax

@@ -7,8 +7,7 @@
 // One tile = 2048 consecutive sequences of one block.  The block-level part of the scan (the prefix of each tile
 // inside its block) is computed first by k_tilesum, so tiles are independent here: static assignment,
 // no ticket, no look-back.  dst[] and lsrc[] are never written to memory.  Matches of depths 1 .. list_hi get list
-// entries; strategy SPAN (shallow streams) sets list_hi = max_depth - 1 and copies the last depth straight from the
-// stream (k_span.cu).
+// entries (list_hi = max_depth whenever this kernel runs).
 #include "common.cuh"
 #include "copy.cuh"
 
@@ -17,8 +16,8 @@ namespace ax {
 struct PreSmem {
     unsigned long long warp_sum[PRE_THREADS / 32];
     uint32_t nloc;                       // entries placed in the tile's sorted list so far
-    uint32_t e_dst[TILE], e_off[TILE], e_g[TILE];   // the tile's matches grouped by depth; e_g = index in the wave list
-    uint16_t e_len[TILE];
+    uint32_t e_dst[TILE_LIST], e_off[TILE_LIST], e_g[TILE_LIST];   // the tile's matches grouped by depth; e_g = index in the wave list
+    uint16_t e_len[TILE_LIST];
     // followed in dynamic shared memory by the depth bins, sized to the stream (pre_bins(max_depth) entries each):
     //   uint32_t cnt[]    per-depth count inside the tile
     //   uint32_t gbase[]  per-depth start in the wave list reserved for this tile
@@ -54,7 +53,7 @@ __global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pre(Params 
         const unsigned long long tile_prefix = P.tile_state[tile];
         const BlockDesc B = P.blocks[b];
         const uint32_t t_in_blk = tile - B.tile_base;
-        const uint32_t j0 = t_in_blk * TILE + tid * PRE_ITEMS;          // first sequence of this thread
+        const uint32_t j0 = t_in_blk * TILE_LIST + tid * PRE_ITEMS;          // first sequence of this thread
         // ---- a2: parse (16-byte loads; streams are padded to 16 bytes, entries past n_seq are masked)
         Seq8 q;
         load_seq8(q, P.comp, B, j0, true);
@@ -110,7 +109,6 @@ __global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pre(Params 
                 else if (dp[k] == 0 || dp[k] > P.max_depth) { raise_fault(P.status, F_DEPTH, b); m = false; }
             }
             if (m) { const uint32_t dist = mdst - of[k]; src_bytes += l[k] < dist ? l[k] : dist; }
-            if (dp[k] > P.list_hi) m = false;                // strategy SPAN: the last depth is copied by k_span, no list entry
             of[k] = m ? of[k] : 0xFFFFFFFFu;
             c[k] = mdst;
             pos += l[k];

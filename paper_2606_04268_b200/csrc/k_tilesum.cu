@@ -1,6 +1,6 @@
 // k_tilesum.cu — step a3, block level: the exclusive prefix of (cmd+len, cmd) of every tile inside its block, i.e. the
 // sequential walk of PAPER.md:53 ("processes cmd[] in sequence") restated as a two-level scan: this kernel produces one
-// prefix per tile (2048 sequences), the consumers (k_pre, k_span) scan inside the tile with warp shuffles.  Also writes
+// prefix per tile (Params::tile sequences), the consumers (k_pre, k_pass, k_chain) scan inside the tile with warp shuffles.  Also writes
 // the tile -> block map and checks invariant I1 (the block's tokens sum to raw_len, its literal runs to n_lit): every
 // later kernel relies on it — with the totals right, every token's range lies inside its block.
 // One CTA per 1 MB block; each WARP sums whole tiles on its own (all its loads independent), then one
@@ -20,16 +20,15 @@ __global__ void __launch_bounds__(TS_THREADS) k_tilesum(Params P) {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (uint32_t b = blockIdx.x; b < P.n_blocks; b += gridDim.x) {
         const BlockDesc B = P.blocks[b];
-        const uint32_t nt = (B.n_seq + TILE - 1) / TILE;
+        const uint32_t nt = (B.n_seq + P.tile - 1) / P.tile;
         __syncthreads();
         if (tid == 0) s_carry = 0;
         for (uint32_t t0 = 0; t0 < nt; t0 += TS_CHUNK) {
             const uint32_t tn = nt - t0 < TS_CHUNK ? nt - t0 : TS_CHUNK;
             for (uint32_t t = warp; t < tn; t += TS_WARPS) {
                 unsigned long long s = 0;
-#pragma unroll
-                for (int r = 0; r < TILE / 256; ++r) {
-                    const uint32_t j0 = (t0 + t) * TILE + r * 256 + lane * 8;
+                for (uint32_t r = 0; r < P.tile / 256; ++r) {                // (tile is a multiple of 256)
+                    const uint32_t j0 = (t0 + t) * P.tile + r * 256 + lane * 8;
                     if (j0 < B.n_seq) {
                         const uint4 vc = *reinterpret_cast<const uint4*>(P.comp + B.cmd_off + 2ull * j0);
                         const uint4 vl = *reinterpret_cast<const uint4*>(P.comp + B.len_off + 2ull * j0);

@@ -13,12 +13,7 @@ from streams import build_stream, flatten_blocks, py_decode, py_depths, random_b
 pytestmark = pytest.mark.gpu
 
 STRATS = [ax.WAVES_LAUNCH, ax.WAVES_GRAPH, ax.WAVES_PERSISTENT]       # wave lists for every depth, three ways of sequencing
-ALL_STRATS = STRATS + [ax.WAVES_SPAN]                                 # + last depth by the streaming span pass (k_span)
-
-
-def span_ok(comp):
-    """Strategy SPAN needs at least one match depth (header offset 40: max_depth)."""
-    return int(np.frombuffer(comp[40:44].tobytes(), "<u4")[0]) >= 1
+ALL_STRATS = STRATS + [ax.WAVES_PASSES]                               # + one streaming pass per depth (shallow streams only)
 
 
 def chain_ok(comp):
@@ -32,8 +27,7 @@ def passes_ok(comp):
 
 
 def strats_for(comp):
-    return STRATS + ([ax.WAVES_SPAN] if span_ok(comp) else []) + ([ax.WAVES_CHAIN] if chain_ok(comp) else []) + \
-        ([ax.WAVES_PASSES] if passes_ok(comp) else [])
+    return STRATS + ([ax.WAVES_CHAIN] if chain_ok(comp) else []) + ([ax.WAVES_PASSES] if passes_ok(comp) else [])
 
 
 def gpu_decode(comp, strategy=0, check=True):
@@ -98,7 +92,7 @@ def test_periodic_overlap(k, n):
         blocks = [[(lead + pat, n, len(lead))]]
         s = build_stream(blocks, 1 << 17, flags=5)
         exp = lead + (pat * (n // k + 2))[:k + n]
-        for strat in (ax.WAVES_SPAN, ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, strat
 
@@ -114,7 +108,7 @@ def test_long_copies_all_alignments():
             seqs.append((lit, 33 + 7 * sa + da, 100 + sa))
     blocks = [seqs]
     s = build_stream(blocks, 1 << 20, flags=5)                                  # every source is literal: I3 holds
-    for strat in (ax.WAVES_SPAN, ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+    for strat in (ax.WAVES_CHAIN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
         got, _ = gpu_decode(s, strat)
         assert got.tobytes() == py_decode(blocks), strat
 
@@ -180,7 +174,7 @@ def test_phases_and_replay():
     from paper_2606_04268_b200.torch_io import Decoder
     raw = workloads.generate("text", 2 << 20, 9)
     comp = oracle.encode(raw, depth_limit=4)
-    for strat in ALL_STRATS + [ax.WAVES_CHAIN, ax.WAVES_PASSES]:
+    for strat in ALL_STRATS + [ax.WAVES_CHAIN]:
         d = Decoder(comp, 0, strat)
         d.run(ax.PHASE_PRE)
         d.run(ax.PHASE_MATCH)
@@ -257,7 +251,7 @@ def test_device_faults_are_flagged_not_fatal():
         t[off:off + len(vals)] = np.frombuffer(bytes(vals), np.uint8)
         return t
     assert run(s)["rc"] == 0
-    for strat in ALL_STRATS + [ax.WAVES_CHAIN, ax.WAVES_PASSES]:
+    for strat in ALL_STRATS + [ax.WAVES_CHAIN]:
         st = run(mut(po, [9]), strat)                         # cmd[0] 8 -> 9: block no longer sums
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_BLOCK_SUM and st["fault_block"] == 0
         st = run(mut(po + 48 + 4, [200]), strat)              # off[1] >= mdst
@@ -271,7 +265,7 @@ def test_device_faults_are_flagged_not_fatal():
     two = build_stream([[(b"abcdefgh", 8, 0), (b"WX", 8, 8), (b"z", 5, 26)]], 32)   # depths 1,2,1
     t = two.copy()
     t[po + 32 + 2] = 1                                        # dep[1] 2 -> 1: counts disagree with the histogram
-    for strat in [0] + ALL_STRATS + [ax.WAVES_PASSES]:
+    for strat in [0] + ALL_STRATS:
         st = run(t, strat)
         assert st["rc"] == ax.E_STREAM and st["fault_flags"] & ax.F_DEPTH
 
@@ -330,9 +324,9 @@ def test_full_size(case, full_streams):
 
 
 @pytest.mark.parametrize("seed", range(4))
-def test_fuzz_shallow_streams_span(seed):
+def test_fuzz_shallow_streams_passes(seed):
     """Encoder-free fuzz restricted to shallow depths (sources drawn from literal bytes or shallow matches): the
-    span pass sees random overlaps, tile-straddling sources, multi-tile blocks and pieces shorter than a word."""
+    per-depth passes see random overlaps, tile-straddling sources and multi-tile blocks."""
     rng = np.random.default_rng(900 + seed)
     for bs, nb in ((64, 40), (4096, 6), (1 << 16, 3), (1 << 18, 2)):
         blocks = random_blocks(rng, bs, nb, max_len=60 if bs < 4096 else 400, max_lit=12 if bs < 4096 else 60, p_match=0.7)
@@ -352,7 +346,7 @@ def test_fuzz_shallow_streams_span(seed):
             nblocks.append(nb_)
         assert py_decode(nblocks) == exp
         s = build_stream(nblocks, bs, min_match=1)
-        for strat in (ax.WAVES_SPAN, ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
+        for strat in (ax.WAVES_PASSES, ax.WAVES_LAUNCH, ax.WAVES_PERSISTENT):
             got, _ = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, nb, seed, strat)
 
@@ -396,7 +390,7 @@ def test_understated_depth_is_undefined_but_in_bounds():
         oracle.validate(s)
     assert e.value.name == "E_I4"
     G = 4096
-    for strat in STRATS + [ax.WAVES_SPAN, ax.WAVES_PASSES]:
+    for strat in ALL_STRATS:
         p = ax.Plan(s.ctypes.data, s.size, 0)
         p.set_strategy(strat)
         cd = torch.from_numpy(s).cuda()
@@ -491,7 +485,7 @@ def test_sparse_depths_empty_waves():
         deps2, _ = py_depths(nblocks, bs)
         doubled = [[2 * d for d in dd] for dd in deps2]
         s = build_stream(nblocks, bs, deps=doubled, min_match=1)
-        for strat in [0] + ALL_STRATS + [ax.WAVES_PASSES]:
+        for strat in [0] + ALL_STRATS:
             got, st = gpu_decode(s, strat)
             assert got.tobytes() == exp, (bs, strat)
             assert st["max_depth"] % 2 == 0
