@@ -81,7 +81,7 @@ extern "C" const char* aceapex_strerror(int code) {
 //   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5.5 us + 21 ps per match copied from a list
 //   PERSISTENT  the same lists, one cooperative kernel: ~4 us of grid barrier + fence drain + straggler wait per depth
 //   CHAIN       (FLATTENED streams only) literal pass 3.1 ps/seq, then one pass whose time is the larger of the block chain
-//               (one ~7.1 us hop per 1 MB block) and its issue-bound throughput (26 ps/seq)
+//               (one ~6.5 us hop per 1 MB block) and its issue-bound throughput (26 ps/seq)
 // PASSES is limited to PASS_MAX_DEPTH waves.
 static int choose_strategy(const aceapex_plan_t* p) {
     if (p->max_depth == 0) return ACEAPEX_WAVES_LAUNCH;
@@ -91,7 +91,7 @@ static int choose_strategy(const aceapex_plan_t* p) {
     const double t_lists = 14.5e-6 * seq + 21e-6 * m;                           // microseconds
     const double t_launch = t_lists + 5.5 * waves, t_persist = t_lists + 4.0 * waves + 8.0;
     const double t_passes = p->max_depth <= PASS_MAX_DEPTH ? 6.1e-6 * seq + p->max_depth * (3.6e-6 * seq + 3.0) + 8.8e-6 * m : 1e300;
-    const double hop = 7.1 * p->n_blocks, thr = 26e-6 * seq;
+    const double hop = 6.5 * p->n_blocks, thr = 26e-6 * seq;
     const double t_chain = (p->flags & FLAG_FLATTENED) ? 3.1e-6 * seq + (hop > thr ? hop : thr) + 10.0 : 1e300;
     int best = ACEAPEX_WAVES_LAUNCH; double t = t_launch;
     if (t_persist < t) { best = ACEAPEX_WAVES_PERSISTENT; t = t_persist; }

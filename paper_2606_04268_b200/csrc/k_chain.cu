@@ -5,9 +5,10 @@
 // order; a tile that holds a match of depth > 1 with a source before its block waits until every earlier block is
 // completely written (a7: per-block completion counts + a frontier word instead of one grid barrier per depth —
 // PAPER.md:224 "synchronization-bound"); dep[] is used only to skip the wait (dep == 1: all sources are literals).
-// Per tile (512 sequences of one block, 256 threads, 4 CTAs per SM):
+// Per tile (512 sequences of one block, 256 threads, 3 CTAs per SM):
 //   a2  the tile's cmd[] / len[] / dep[] / off[] slices and its slice of lit[] arrive in shared memory by 1-D bulk TMA
-//       (cp.async.bulk + mbarrier); the next tile's descriptor is fetched by one thread (cp.async) meanwhile
+//       (cp.async.bulk + mbarrier), two stages: the tile after next is in flight; its descriptor is fetched by one thread
+//       (cp.async) meanwhile
 //   a3  scan inside the tile: each thread sums 2 CONSECUTIVE sequences, warp shuffles + one barrier give every token's
 //       output position and literal offset (the tile's prefix inside its block comes from k_tilesum), kept in shared memory
 //   a6  then thread t takes tokens t, t+256 (neighbouring lanes = neighbouring tokens: neighbouring sources share L1
@@ -19,8 +20,8 @@
 //         assemble         every match is written into the image with naturally aligned 1/2/4-byte stores (each byte has
 //                          one owner: no merge, no zero fill), periodic if it overlaps its source (Q3); matches
 //                          up to 32 bytes by one thread, longer ones by the whole warp
-//       and the image goes to global memory with one bulk TMA store (16-byte chunks; <= 15 head / tail bytes by byte
-//       stores).  Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight
+//       and the image goes to global memory with coalesced 16-byte vector stores (<= 15 head / tail bytes by byte stores;
+//       measured against one bulk TMA store + its completion wait: 7.2 vs 7.7 ms on fastq1g — the wait is on the chain).  Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight
 //       to global memory instead (their literal runs are there already: the literal scatter ran before).
 // Rewriting a literal byte with its own value while another CTA reads it as a match source is harmless: a reader sees the
 // old or the new copy of the same value.
@@ -34,7 +35,8 @@ constexpr int SP_PER = 2;                            // tokens per thread (measu
                                                      // and a 512-sequence tile spreads a block's ~370 tiles over all SMs: 7.1 us)
 constexpr int SP_THREADS = TILE / SP_PER;            // 256
 constexpr int SP_WARPS = SP_THREADS / 32;
-constexpr int SP_OCC = 4;                            // CTAs per SM: 592 resident tiles = 1.6 blocks of a stream of 5.6-byte matches
+constexpr int SP_OCC = 3;                            // CTAs per SM (85 registers per thread: measured 7.7 / 8.05 / 10.3 ms on fastq1g
+                                                     // for 3 / 4 / 5 CTAs — the register cap costs more than residency gains)
 constexpr uint32_t SP_STRM = TILE * 10u;             // cmd | len | dep (2 B each) | off (4 B) per sequence
 constexpr uint32_t SP_O_LEN = TILE * 2u, SP_O_DEP = TILE * 4u, SP_O_OFF = TILE * 6u;
 constexpr uint32_t SP_IMG = 10 * TILE;               // image capacity in bytes (a text / FASTQ tile of 512 sequences spans ~3 KB)
@@ -63,15 +65,15 @@ struct alignas(16) TileFetch {
 static_assert(sizeof(BlockDesc) == 64, "BlockDesc travels as four 16-byte cp.async");
 
 struct SpanSmem {
-    alignas(128) uint8_t strm[SP_STRM];
-    alignas(128) uint8_t slit[SP_LIT + 32];
+    alignas(128) uint8_t strm[2][SP_STRM];           // two stages: the tile after next is in flight while this one is processed
+    alignas(128) uint8_t slit[2][SP_LIT + 32];
     alignas(16) uint32_t pos[TILE];                  // absolute output position of token j's literal run; later its source address
     alignas(16) uint32_t lpos[TILE];                 // offset of token j's literal run inside the block's lit[]; later its copy info
     alignas(16) unsigned long long x0[TILE], x1[TILE], x2[TILE], x3[TILE], x4[TILE];   // the aligned words holding token j's source bytes
     alignas(128) uint8_t img[SP_IMG + 64];
-    alignas(8) unsigned long long mbar;
+    alignas(8) unsigned long long mbar[2];
     TileFetch fetch;                                 // (thread 0) descriptor of the next tile
-    TileMeta meta;
+    TileMeta meta[2];
     unsigned long long warp_sum[SP_WARPS];
     uint32_t img_end;                                // absolute end of the span held by the image
 };
@@ -97,14 +99,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t pari
 __device__ __forceinline__ void bulk_load(void* smem, const void* gmem, uint32_t bytes, unsigned long long* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(smem)), "l"(gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-// 1-D bulk TMA: shared -> global, tracked by the thread's bulk async-group
-__device__ __forceinline__ void bulk_store(void* gmem, const void* smem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gmem), "r"(smem_u32(smem)), "r"(bytes) : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-}
-__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem)), "l"(gmem) : "memory");
@@ -133,36 +127,24 @@ __device__ __forceinline__ void fetch_step2(const Params& P, TileFetch& F) {
 // The tile's stream slices (and its slice of lit[]) -> the stage, and its TileMeta (one elected thread).  Slices start on
 // 4096-byte multiples of 16-byte aligned streams and are padded to 16 bytes inside the payload (docs/FORMAT.md), so sizes
 // round up to 16 safely.  The arrive (release) orders the meta stores before any waiter's reads (acquire).
-__device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, uint32_t tile, const TileFetch& F) {
+__device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, uint32_t tile, const TileFetch& F, uint32_t st) {
     const uint32_t j0 = (tile - F.B.tile_base) * TILE;
     const uint32_t left = F.B.n_seq - j0, n = left < (uint32_t)TILE ? left : (uint32_t)TILE;
     const uint32_t lit_lo = (uint32_t)F.pre, lit_hi = j0 + n < F.B.n_seq ? (uint32_t)F.pre1 : F.B.n_lit;
     const uint32_t l16 = lit_lo & ~15u;
     const uint32_t lbytes = lit_hi >= lit_lo ? (uint32_t)pad16(lit_hi) - l16 : 0xFFFFFFFFu;
     const bool lit_ok = lbytes <= SP_LIT;
-    TileMeta& M = S.meta;
+    TileMeta& M = S.meta[st];
     M.pre = F.pre; M.lit = P.comp + F.B.lit_off; M.b = F.b; M.blk_lo = (uint32_t)F.B.out_base; M.nt = n;
     M.blk_tiles = (F.B.n_seq + TILE - 1) / TILE; M.prev_tiles = (F.prev_tiles + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
     const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
-    mbar_expect_tx(&S.mbar, 3 * b2 + b4 + (lit_ok ? lbytes : 0u));
-    bulk_load(S.strm, P.comp + F.B.cmd_off + 2ull * j0, b2, &S.mbar);
-    bulk_load(S.strm + SP_O_LEN, P.comp + F.B.len_off + 2ull * j0, b2, &S.mbar);
-    bulk_load(S.strm + SP_O_DEP, P.comp + F.B.dep_off + 2ull * j0, b2, &S.mbar);
-    bulk_load(S.strm + SP_O_OFF, P.comp + F.B.off_off + 4ull * j0, b4, &S.mbar);
-    if (lit_ok && lbytes) bulk_load(S.slit, P.comp + F.B.lit_off + l16, lbytes, &S.mbar);
+    mbar_expect_tx(&S.mbar[st], 3 * b2 + b4 + (lit_ok ? lbytes : 0u));
+    bulk_load(S.strm[st], P.comp + F.B.cmd_off + 2ull * j0, b2, &S.mbar[st]);
+    bulk_load(S.strm[st] + SP_O_LEN, P.comp + F.B.len_off + 2ull * j0, b2, &S.mbar[st]);
+    bulk_load(S.strm[st] + SP_O_DEP, P.comp + F.B.dep_off + 2ull * j0, b2, &S.mbar[st]);
+    bulk_load(S.strm[st] + SP_O_OFF, P.comp + F.B.off_off + 4ull * j0, b4, &S.mbar[st]);
+    if (lit_ok && lbytes) bulk_load(S.slit[st], P.comp + F.B.lit_off + l16, lbytes, &S.mbar[st]);
 }
-// The same slices pulled into L2 ahead of time (the stage is single-buffered: the load proper is issued when the
-// previous tile is done with it and then finds its bytes in L2 instead of DRAM).
-__device__ __forceinline__ void prefetch_tile_l2(const Params& P, uint32_t tile, const TileFetch& F) {
-    const uint32_t j0 = (tile - F.B.tile_base) * TILE;
-    const uint32_t left = F.B.n_seq - j0, n = left < (uint32_t)TILE ? left : (uint32_t)TILE;
-    const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
-    bulk_prefetch_l2(P.comp + F.B.cmd_off + 2ull * j0, b2);
-    bulk_prefetch_l2(P.comp + F.B.len_off + 2ull * j0, b2);
-    bulk_prefetch_l2(P.comp + F.B.dep_off + 2ull * j0, b2);
-    bulk_prefetch_l2(P.comp + F.B.off_off + 4ull * j0, b4);
-}
-
 // bytes [sb, sb+16) of the 24-byte value (x0 | x1 << 64 | x2 << 128), sb in 0..7
 __device__ __forceinline__ V16 extract16(unsigned long long x0, unsigned long long x1, unsigned long long x2, uint32_t sb) {
     const uint32_t s = sb * 8u;
@@ -183,32 +165,37 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
     uint32_t tile = blockIdx.x;
     TileFetch& F = S.fetch;
     if (tid == 0) {
-        mbar_init(&S.mbar, 1);
+        mbar_init(&S.mbar[0], 1); mbar_init(&S.mbar[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        if (tile < P.n_tiles) {
-            fetch_step1(P, F, tile); fetch_step2(P, F);
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
-            issue_tile_loads(P, S, tile, F);
+        for (uint32_t i = 0; i < 2u; ++i) {                               // the first two tiles of this CTA, one per stage
+            const uint32_t t = tile + i * gridDim.x;
+            if (t < P.n_tiles) {
+                fetch_step1(P, F, t); fetch_step2(P, F);
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                issue_tile_loads(P, S, t, F, i);
+            }
         }
     }
     __syncthreads();
     uint32_t n_copied = 0;
     unsigned long long src_bytes = 0;                // M_src (this pass is the one that validates every match)
-    uint16_t* const s_cmd = reinterpret_cast<uint16_t*>(S.strm);
-    uint16_t* const s_len = reinterpret_cast<uint16_t*>(S.strm + SP_O_LEN);
-    uint16_t* const s_dep = reinterpret_cast<uint16_t*>(S.strm + SP_O_DEP);
-    uint32_t* const s_off = reinterpret_cast<uint32_t*>(S.strm + SP_O_OFF);
 
     for (uint32_t it = 0; tile < P.n_tiles; ++it, tile += gridDim.x) {
-        const uint32_t next = tile + gridDim.x;
+        const uint32_t st = it & 1u;
+        const uint32_t next = tile + 2u * gridDim.x;                      // the tile that takes this stage over when this one is done
         const bool has_next = next < P.n_tiles;
         if (tid == 0 && has_next) fetch_step1(P, F, next);                 // consumed after the scan below
-        // ---- a2: the tile's slices have landed
-        mbar_wait(&S.mbar, it & 1u);
-        const unsigned long long pre = S.meta.pre;
-        const uint8_t* const lit = S.meta.lit;
-        const uint32_t b = S.meta.b, blk_lo = S.meta.blk_lo, nt = S.meta.nt, blk_tiles = S.meta.blk_tiles, prev_tiles = S.meta.prev_tiles;
-        const uint8_t* const lsrc_base = S.meta.lit_ok ? S.slit - S.meta.lit16 : lit;   // byte x of the block's lit[] is lsrc_base[x]
+        // ---- a2: the tile's slices have landed (they were requested one tile ago)
+        mbar_wait(&S.mbar[st], (it >> 1) & 1u);
+        const TileMeta& M = S.meta[st];
+        const unsigned long long pre = M.pre;
+        const uint8_t* const lit = M.lit;
+        const uint32_t b = M.b, blk_lo = M.blk_lo, nt = M.nt, blk_tiles = M.blk_tiles, prev_tiles = M.prev_tiles;
+        const uint8_t* const lsrc_base = M.lit_ok ? S.slit[st] - M.lit16 : lit;   // byte x of the block's lit[] is lsrc_base[x]
+        uint16_t* const s_cmd = reinterpret_cast<uint16_t*>(S.strm[st]);
+        uint16_t* const s_len = reinterpret_cast<uint16_t*>(S.strm[st] + SP_O_LEN);
+        uint16_t* const s_dep = reinterpret_cast<uint16_t*>(S.strm[st] + SP_O_DEP);
+        uint32_t* const s_off = reinterpret_cast<uint32_t*>(S.strm[st] + SP_O_OFF);
         const uint32_t A0 = blk_lo + (uint32_t)(pre >> 32);               // absolute start of the tile's span
         const uint32_t img_org = A0 & ~15u;                               // absolute position of image byte 0
         // ================= phase S (thread t owns sequences 4t .. 4t+3): a3 scan, token validation
@@ -233,10 +220,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
             if (lane >= (uint32_t)d) inc += t;
         }
         if (lane == 31) S.warp_sum[warp] = inc;
-        if (tid == 0) {
-            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the previous tile's store has read the image
-            S.img_end = A0;
-        }
+        if (tid == 0) S.img_end = A0;
         const bool must_wait = __syncthreads_or(wait_src) != 0;           // barrier 1
         {
             unsigned long long wpre = 0;
@@ -320,7 +304,10 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
                     __nanosleep(400);                                     // not next in line: keep the hot lines' queues short
                 }
                 if (v < b) {
-                    do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory"); } while (v < prev_tiles);
+                    for (;;) {
+                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + (b - 1u)) : "memory");
+                        if (v >= prev_tiles) break;
+                    }
                 }
                 asm volatile("fence.acq_rel.gpu;" ::: "memory");
             }
@@ -344,7 +331,6 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
         asm volatile("cp.async.wait_group 0;" ::: "memory");
-        if (tid == 0 && has_next) prefetch_tile_l2(P, next, F);
         // ================= phase M: a6, every match into the image (or, beyond its capacity, straight to global memory).
         // The thread's tokens are unrolled so that their dependent shift / store chains interleave.
         bool any_long = false;
@@ -387,43 +373,35 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
                 }
             }
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // generic-proxy image writes -> visible to the bulk store
         __syncthreads();                                                  // barrier 4: image complete, stage free
-        if (tid < 32u) {
-            // ---- write the image out: 16-byte chunks by one bulk TMA store, the partial chunks at both ends by byte stores
+        {
+            // ---- write the image out: 16-byte chunks by plain coalesced vector stores, the partial chunks at both ends by bytes
             const uint32_t E = S.img_end;
             const uint32_t c0 = (A0 + 15u) & ~15u, c1 = E & ~15u;
-            if (tid == 0 && c1 > c0) bulk_store(P.out + c0, S.img + (c0 - img_org), c1 - c0);
-            // the next tile's slices start travelling while this tile's image is stored
-            if (tid == 0 && has_next) issue_tile_loads(P, S, next, F);
+            if (c1 > c0) {
+                const uint4* src = reinterpret_cast<const uint4*>(S.img + (c0 - img_org));
+                uint4* dst = reinterpret_cast<uint4*>(P.out + c0);
+                for (uint32_t i = tid; i < ((c1 - c0) >> 4); i += SP_THREADS) dst[i] = src[i];
+            }
+            if (tid == 0 && has_next) issue_tile_loads(P, S, next, F, st);   // the stage is free
             const uint32_t he = c0 < E ? c0 : E;                          // head bytes [A0, he)
-            if (tid < 16u && A0 + tid < he) P.out[A0 + tid] = S.img[A0 + tid - img_org];
-            if (tid >= 16u && c1 >= c0) {                                 // tail bytes [c1, E)
-                const uint32_t a = c1 + (tid - 16u);
+            if (tid >= 32u && tid < 48u && A0 + (tid - 32u) < he) P.out[A0 + (tid - 32u)] = S.img[A0 + (tid - 32u) - img_org];
+            if (tid >= 48u && tid < 64u && c1 >= c0) {                    // tail bytes [c1, E)
+                const uint32_t a = c1 + (tid - 48u);
                 if (a < E) P.out[a] = S.img[a - img_org];
             }
-            {
-                // publish: the tile's bytes (bulk store complete, head / tail / direct stores ordered by barrier 4 and the
-                // warp barrier) happen before the release-add; the tile that completes block b moves the frontier, in
-                // block order (blocks whose tiles never had to wait may finish early).
-                if (tid == 0) {
-                    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-                    asm volatile("fence.proxy.async;" ::: "memory");
-                }
-                __syncwarp();
-                if (tid == 0) {
-                    uint32_t old;
-                    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
-                    if (old + 1u == blk_tiles) {                          // block b complete: move the frontier word, in block order
-                        uint32_t v;
-                        do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory"); } while (v < b);
-                        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(P.chain_sync), "r"(b + 1u) : "memory");
-                    }
+            __syncthreads();                                              // barrier 5: every store of the tile is issued
+            if (tid == 0) {
+                uint32_t old;
+                asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
+                if (old + 1u == blk_tiles) {
+                    uint32_t v;
+                    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory"); } while (v < b);
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(P.chain_sync), "r"(b + 1u) : "memory");
                 }
             }
         }
     }
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 #pragma unroll
     for (int d = 16; d; d >>= 1) n_copied += __shfl_xor_sync(0xFFFFFFFFu, n_copied, d);
     if (lane == 0 && n_copied) atomicAdd(&P.status->n_final, n_copied);
