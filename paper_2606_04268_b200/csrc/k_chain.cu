@@ -67,8 +67,6 @@ static_assert(sizeof(BlockDesc) == 64, "BlockDesc travels as four 16-byte cp.asy
 struct SpanSmem {
     alignas(128) uint8_t strm[2][SP_STRM];           // two stages: the tile after next is in flight while this one is processed
     alignas(128) uint8_t slit[2][SP_LIT + 32];
-    alignas(16) uint32_t pos[TILE];                  // absolute output position of token j's literal run; later its source address
-    alignas(16) uint32_t lpos[TILE];                 // offset of token j's literal run inside the block's lit[]; later its copy info
     alignas(16) unsigned long long x0[TILE], x1[TILE], x2[TILE], x3[TILE], x4[TILE];   // the aligned words holding token j's source bytes
     alignas(128) uint8_t img[SP_IMG + 64];
     alignas(8) unsigned long long mbar[2];
@@ -198,101 +196,94 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
         uint32_t* const s_off = reinterpret_cast<uint32_t*>(S.strm[st] + SP_O_OFF);
         const uint32_t A0 = blk_lo + (uint32_t)(pre >> 32);               // absolute start of the tile's span
         const uint32_t img_org = A0 & ~15u;                               // absolute position of image byte 0
-        // ================= phase S (thread t owns sequences 4t .. 4t+3): a3 scan, token validation
+        // ================= before the wait (needs nothing another block wrote).  Thread t owns sequences 2t and 2t+1 through
+        // every phase: what it learns about them stays in registers, and a token is only ever touched by its own thread.
+        // ---- a3: scan of (cmd+len, cmd) packed as (hi, lo) of one u64
         const uint32_t jt = tid * SP_PER;
-        uint32_t c4[SP_PER], l4[SP_PER], d4[SP_PER], o4[SP_PER];
-#pragma unroll
-        for (int k = 0; k < SP_PER; ++k) {
-            const bool in = jt + k < nt;
-            c4[k] = in ? s_cmd[jt + k] : 0u; l4[k] = in ? s_len[jt + k] : 0u; d4[k] = in ? s_dep[jt + k] : 0u; o4[k] = in ? s_off[jt + k] : 0u;
+        uint32_t c[SP_PER], l[SP_PER], d[SP_PER], o[SP_PER];
+        {
+            uint32_t vc = 0, vl = 0, vd = 0; uint2 vo = make_uint2(0u, 0u);
+            if (jt < nt) {
+                vc = *reinterpret_cast<const uint32_t*>(s_cmd + jt); vl = *reinterpret_cast<const uint32_t*>(s_len + jt);
+                vd = *reinterpret_cast<const uint32_t*>(s_dep + jt); vo = *reinterpret_cast<const uint2*>(s_off + jt);
+            }
+            c[0] = vc & 0xFFFFu; c[1] = vc >> 16; l[0] = vl & 0xFFFFu; l[1] = vl >> 16; d[0] = vd & 0xFFFFu; d[1] = vd >> 16;
+            o[0] = vo.x; o[1] = vo.y;
+            if (jt + 1u >= nt) { c[1] = 0; l[1] = 0; }                    // the tail shares its words with nothing: mask
         }
         unsigned long long tsum = 0;
         bool wait_src = false;                       // a match deeper than 1 reads an earlier block
 #pragma unroll
         for (int k = 0; k < SP_PER; ++k) {
-            tsum += ((unsigned long long)(c4[k] + l4[k]) << 32) | c4[k];
-            wait_src |= l4[k] != 0 && o4[k] < blk_lo && d4[k] != 1u;
+            tsum += ((unsigned long long)(c[k] + l[k]) << 32) | c[k];
+            wait_src |= l[k] != 0 && o[k] < blk_lo && d[k] != 1u;
         }
         unsigned long long inc = tsum;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-            if (lane >= (uint32_t)d) inc += t;
+        for (int dd = 1; dd < 32; dd <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, inc, dd);
+            if (lane >= (uint32_t)dd) inc += t;
         }
         if (lane == 31) S.warp_sum[warp] = inc;
         if (tid == 0) S.img_end = A0;
         const bool must_wait = __syncthreads_or(wait_src) != 0;           // barrier 1
-        {
-            unsigned long long wpre = 0;
+        unsigned long long wpre = 0;
 #pragma unroll
-            for (int w = 0; w < SP_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
-            const unsigned long long ex = pre + wpre + (inc - tsum);
-            uint32_t p = blk_lo + (uint32_t)(ex >> 32), ls = (uint32_t)ex;   // this thread's first token: position, literal offset
-            uint32_t ps[SP_PER], lp[SP_PER];
-            uint32_t bad_src = 0, bad_dep = 0, fit_end = 0;
+        for (int w = 0; w < SP_WARPS; ++w) if (w < (int)warp) wpre += S.warp_sum[w];
+        const unsigned long long ex = pre + wpre + (inc - tsum);
+        // ---- token validation (I2, depth range, I3), literal runs into the image, every match reduced to what its copy needs:
+        //   pp   destination            sa   source address (aligned down to 8 if one thread copies the match)
+        //   inf  len (16 bits) | source byte phase (3) | period if the source overlaps, else 0 (4) | in image | by one thread
+        uint32_t pp[SP_PER], sa[SP_PER], inf[SP_PER], ps[SP_PER], lp[SP_PER];
+        {
+            uint32_t p = blk_lo + (uint32_t)(ex >> 32), ls = (uint32_t)ex, fit_end = 0;
+            bool bad_src = false, bad_dep = false, long_lit = false;
 #pragma unroll
             for (int k = 0; k < SP_PER; ++k) {
                 ps[k] = p; lp[k] = ls;
-                const uint32_t mdst = p + c4[k];
-                if (l4[k]) {                                               // token validation (I2, depth range, I3)
-                    if (o4[k] >= mdst || l4[k] < P.min_match) bad_src |= 1u << k;
-                    else if (d4[k] == 0 || d4[k] > P.max_depth) bad_dep |= 1u << k;
-                    else if (o4[k] >= blk_lo && d4[k] != 1u) bad_dep |= 1u << k;   // an in-block source that is not literal
+                const uint32_t mdst = p + c[k], len = l[k];
+                const bool in_img = mdst + len - img_org <= SP_IMG;       // tokens are monotone: a prefix of the tile fits the image
+                pp[k] = mdst; inf[k] = in_img ? 1u << 23 : 0u; sa[k] = 0;
+                if (len) {
+                    if (o[k] >= mdst || len < P.min_match) bad_src = true;
+                    else if (d[k] == 0 || d[k] > P.max_depth || (o[k] >= blk_lo && d[k] != 1u)) bad_dep = true;   // (in-block source: literal only)
+                    else {
+                        const uint32_t dist = mdst - o[k];
+                        const bool ovl = dist < len;
+                        const bool by_thread = len <= SP_SHORT || (len <= SP_SHORT2 && !ovl);
+                        sa[k] = by_thread ? (o[k] & ~7u) : o[k];
+                        inf[k] |= len | (o[k] & 7u) << 16 | (ovl && by_thread ? dist : 0u) << 19 | (by_thread ? 1u << 26 : 0u);
+                        ++n_copied; src_bytes += ovl ? dist : len;
+                    }
                 }
-                p = mdst + l4[k]; ls += c4[k];
-                if (p - img_org <= SP_IMG) fit_end = p;                   // tokens are monotone: a prefix of the tile fits the image
+                if (c[k] && in_img) {
+                    if (c[k] <= SP_SHORT) place16(S.img + (p - img_org), load16(lsrc_base + ls, c[k]), c[k]);
+                    else long_lit = true;
+                }
+                p = mdst + len;
+                ls += c[k];
+                if (in_img) fit_end = p;
             }
-#pragma unroll
-            for (int k = 0; k < SP_PER; ++k) if (jt + k < nt) { S.pos[jt + k] = ps[k]; S.lpos[jt + k] = lp[k]; }
-            if (bad_src | bad_dep) {                                      // a faulty match is flagged and skipped: its bytes stay a hole
-#pragma unroll
-                for (int k = 0; k < SP_PER; ++k) if ((bad_src | bad_dep) & (1u << k)) s_len[jt + k] = 0;
-                if (bad_src) raise_fault(P.status, F_SOURCE, b);
-                if (bad_dep) raise_fault(P.status, F_DEPTH, b);
-            }
+            if (bad_src) raise_fault(P.status, F_SOURCE, b);              // a faulty match is flagged and skipped: its bytes stay a hole
+            if (bad_dep) raise_fault(P.status, F_DEPTH, b);
             fit_end = __reduce_max_sync(0xFFFFFFFFu, fit_end);
             if (lane == 0 && fit_end) atomicMax(&S.img_end, fit_end);
+            if (__any_sync(0xFFFFFFFFu, long_lit)) {                      // long literal runs: the whole warp copies each
+#pragma unroll
+                for (int k = 0; k < SP_PER; ++k) {
+                    uint32_t m = __ballot_sync(0xFFFFFFFFu, c[k] > SP_SHORT && ((inf[k] >> 23) & 1u));
+                    while (m) {
+                        const int sl = __ffs(m) - 1; m &= m - 1;
+                        const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, ps[k], sl), s2 = __shfl_sync(0xFFFFFFFFu, lp[k], sl), n2 = __shfl_sync(0xFFFFFFFFu, c[k], sl);
+                        warp_copy(S.img + (d2 - img_org), lit + s2, n2, lane);
+                    }
+                }
+            }
         }
         if (tid == 0 && has_next) fetch_step2(P, F);                       // (its block index has arrived by now)
-        __syncthreads();                                                  // barrier 2: pos[] / lpos[] / cleared len[] visible
-        // ================= phase L (thread t takes tokens t, t + SP_THREADS, ...; so do phases G and M: a token is handled
-        // by ONE thread from here on, which is why they need no barrier between them).  Needs nothing another block wrote:
-        // literal runs go into the image, and each match is reduced to what the copy needs —
-        //   pos[j]  <- aligned source address (short match) / source address (long match)
-        //   lpos[j] <- info: len (16 bits) | source byte phase (3) | period if the source overlaps, else 0 (4) | in image |
-        //              copied by one thread (else by the whole warp)
-        //   off[j]  <- match destination
-#pragma unroll 1
-        for (uint32_t j0 = warp * 32u; j0 < nt; j0 += SP_THREADS) {
-            const uint32_t j = j0 + lane;
-            const bool live = j < nt;
-            const uint32_t c = live ? s_cmd[j] : 0u, l = live ? s_len[j] : 0u;
-            const uint32_t ps = live ? S.pos[j] : 0u, lp = live ? S.lpos[j] : 0u;
-            const uint32_t pp = ps + c;
-            const bool in_img = pp + l - img_org <= SP_IMG;
-            if (c && in_img && c <= SP_SHORT) place16(S.img + (ps - img_org), load16(lsrc_base + lp, c), c);
-            uint32_t m = __ballot_sync(0xFFFFFFFFu, c > SP_SHORT && in_img);
-            while (m) {                                                   // long literal runs: the whole warp copies each
-                const int sl = __ffs(m) - 1; m &= m - 1;
-                const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, ps, sl), s2 = __shfl_sync(0xFFFFFFFFu, lp, sl), n2 = __shfl_sync(0xFFFFFFFFu, c, sl);
-                warp_copy(S.img + (d2 - img_org), lit + s2, n2, lane);
-            }
-            if (live) {
-                uint32_t inf = 0, sa = 0;
-                if (l) {
-                    const uint32_t of = s_off[j], dist = pp - of;
-                    const bool ovl = dist < l;
-                    const bool by_thread = l <= SP_SHORT || (l <= SP_SHORT2 && !ovl);
-                    sa = by_thread ? (of & ~7u) : of;
-                    inf = l | (of & 7u) << 16 | (ovl && by_thread ? dist : 0u) << 19 | (in_img ? 1u << 23 : 0u) | (by_thread ? 1u << 26 : 0u);
-                    ++n_copied; src_bytes += ovl ? dist : l;
-                }
-                S.pos[j] = sa; S.lpos[j] = inf; s_off[j] = pp;
-            }
-        }
         if (must_wait) {
-            // a7: every block before this one completely written?  One thread spins on the frontier;
-            // its acquire fence also drops this SM's L1 (CCTL.IVALL), so the loads below see what other SMs wrote.
+            // a7: every block before this one completely written?  One thread spins; its acquire fence also drops this
+            // SM's L1 (CCTL.IVALL), so the loads below see what other SMs wrote.
             if (tid == 0) {
                 // blocks 0 .. b-2: the frontier word (moved by the last tile of every block, in block order, one hop ago);
                 // block b-1: its completion count itself, so that the returning atomic and the frontier store of its last
@@ -304,25 +295,21 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
                     __nanosleep(400);                                     // not next in line: keep the hot lines' queues short
                 }
                 if (v < b) {
-                    for (;;) {
-                        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + (b - 1u)) : "memory");
-                        if (v >= prev_tiles) break;
-                    }
+                    do { asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory"); } while (v < prev_tiles);
                 }
                 asm volatile("fence.acq_rel.gpu;" ::: "memory");
             }
-            __syncthreads();                                              // barrier 3
+            __syncthreads();                                              // barrier 2
         }
-        // ================= phase G: the aligned 8-byte words holding each short match's source travel global -> shared
+        // ================= after the wait.  Gather: the aligned 8-byte words holding each match's source travel global ->
+        // shared (cp.async: no registers held across the round trip, both tokens of the thread in flight at once)
 #pragma unroll
         for (int k = 0; k < SP_PER; ++k) {
-            const uint32_t j = k * SP_THREADS + tid;
-            if (j >= nt) continue;
-            const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
-            if (!((inf >> 26) & 1u)) continue;
-            const uint32_t per = (inf >> 19) & 15u;
-            const uint32_t span = ((inf >> 16) & 7u) + (per ? per : l);
-            const uint8_t* g = P.out + S.pos[j];
+            if (!((inf[k] >> 26) & 1u)) continue;
+            const uint32_t j = k * SP_THREADS + tid;                       // the thread's private slot
+            const uint32_t per = (inf[k] >> 19) & 15u;
+            const uint32_t span = ((inf[k] >> 16) & 7u) + (per ? per : (inf[k] & 0xFFFFu));
+            const uint8_t* g = P.out + sa[k];
             cp_async8(&S.x0[j], g);
             if (span > 8u) cp_async8(&S.x1[j], g + 8);
             if (span > 16u) cp_async8(&S.x2[j], g + 16);
@@ -331,45 +318,37 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
         asm volatile("cp.async.wait_group 0;" ::: "memory");
-        // ================= phase M: a6, every match into the image (or, beyond its capacity, straight to global memory).
-        // The thread's tokens are unrolled so that their dependent shift / store chains interleave.
+        // ---- a6: every match into the image (or, beyond its capacity, straight to global memory)
         bool any_long = false;
 #pragma unroll
         for (int k = 0; k < SP_PER; ++k) {
-            const uint32_t j = k * SP_THREADS + tid;
-            if (j >= nt) continue;
-            const uint32_t inf = S.lpos[j], l = inf & 0xFFFFu;
-            any_long |= l != 0 && !((inf >> 26) & 1u);
-            if ((inf >> 26) & 1u) {
-                const uint32_t pp = s_off[j], per = (inf >> 19) & 15u, sb = (inf >> 16) & 7u;
+            const uint32_t ll = inf[k] & 0xFFFFu;
+            any_long |= ll != 0 && !((inf[k] >> 26) & 1u);
+            if ((inf[k] >> 26) & 1u) {
+                const uint32_t j = k * SP_THREADS + tid, per = (inf[k] >> 19) & 15u, sb = (inf[k] >> 16) & 7u;
                 const unsigned long long y2 = S.x2[j];
                 V16 v = extract16(S.x0[j], S.x1[j], y2, sb);
                 if (per) v = extend_period(v, per);                        // self-overlap: periodic extension (Q3)
-                const uint32_t l0 = l < 16u ? l : 16u;
-                if ((inf >> 23) & 1u) {
-                    place16(S.img + (pp - img_org), v, l0);
-                    if (l > 16u) place16(S.img + (pp - img_org) + 16, extract16(y2, S.x3[j], S.x4[j], sb), l - 16u);
+                const uint32_t l0 = ll < 16u ? ll : 16u;
+                if ((inf[k] >> 23) & 1u) {
+                    place16(S.img + (pp[k] - img_org), v, l0);
+                    if (ll > 16u) place16(S.img + (pp[k] - img_org) + 16, extract16(y2, S.x3[j], S.x4[j], sb), ll - 16u);
                 } else {
-                    store16(P.out + pp, v, l0);
-                    if (l > 16u) store16(P.out + pp + 16, extract16(y2, S.x3[j], S.x4[j], sb), l - 16u);
+                    store16(P.out + pp[k], v, l0);
+                    if (ll > 16u) store16(P.out + pp[k] + 16, extract16(y2, S.x3[j], S.x4[j], sb), ll - 16u);
                 }
             }
         }
         if (__any_sync(0xFFFFFFFFu, any_long)) {                          // long matches: the whole warp copies each
-#pragma unroll 1
-            for (uint32_t j0 = warp * 32u; j0 < nt; j0 += SP_THREADS) {
-                const uint32_t j = j0 + lane;
-                const bool live = j < nt;
-                const uint32_t inf = live ? S.lpos[j] : 0u, l = inf & 0xFFFFu;
-                const uint32_t pp = live ? s_off[j] : 0u, sa = live ? S.pos[j] : 0u;
-                uint32_t m = __ballot_sync(0xFFFFFFFFu, l != 0 && !((inf >> 26) & 1u));
+#pragma unroll
+            for (int k = 0; k < SP_PER; ++k) {
+                uint32_t m = __ballot_sync(0xFFFFFFFFu, (inf[k] & 0xFFFFu) != 0 && !((inf[k] >> 26) & 1u));
                 while (m) {
                     const int sl = __ffs(m) - 1; m &= m - 1;
-                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, pp, sl), o2 = __shfl_sync(0xFFFFFFFFu, sa, sl),
-                                   n2 = __shfl_sync(0xFFFFFFFFu, l, sl), f2 = __shfl_sync(0xFFFFFFFFu, inf, sl);
+                    const uint32_t d2 = __shfl_sync(0xFFFFFFFFu, pp[k], sl), o2 = __shfl_sync(0xFFFFFFFFu, sa[k], sl), f2 = __shfl_sync(0xFFFFFFFFu, inf[k], sl);
                     const bool im2 = (f2 >> 23) & 1u;
                     uint8_t* dst = im2 ? S.img + (d2 - img_org) : P.out + d2;
-                    warp_match(dst, P.out + o2, n2, d2 - o2, !im2, lane);
+                    warp_match(dst, P.out + o2, f2 & 0xFFFFu, d2 - o2, !im2, lane);
                 }
             }
         }
