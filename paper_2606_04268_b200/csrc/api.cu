@@ -17,6 +17,7 @@ cudaError_t pass_configure();
 int pass_max_ctas_per_sm();
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st);
 void launch_pass_reset(const Params& P, cudaStream_t st);
+void launch_litcopy(const Params& P, int grid, cudaStream_t st);
 cudaError_t pre_configure();
 int pre_max_ctas_per_sm(uint32_t max_depth);
 int match_max_ctas_per_sm();
@@ -41,11 +42,12 @@ struct aceapex_plan_s {
     uint32_t flags, block_size, n_blocks, min_match, depth_limit, max_depth;
     uint64_t raw_size, total_seq, total_lit, comp_bytes, n_match;
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
+    uint32_t lit_q_cap;                             // capacity of the long-literal queue
     uint32_t n_tiles_list, n_tiles_stream;          // tiles at TILE_LIST / TILE_STREAM sequences per tile
     // device facts
     int device, n_sm, pre_grid, match_ctas_per_sm, chain_grid, pass_grid;
     // scratch layout (byte offsets)
-    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_chain, o_dst, o_off, o_len, scratch_bytes;
+    size_t o_status, o_wave_off, o_cursor, o_blocks, o_tiles, o_tblk, o_chain, o_litq, o_dst, o_off, o_len, scratch_bytes;
     int strategy_auto, strategy_forced;
     uint32_t last_launches; int last_strategy; bool last_had_match;
     int last_cuda;
@@ -171,6 +173,8 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_tiles = o; o += up256(8ull * p->n_tiles_stream);       // (sized for the finer tiling)
         p->o_tblk = o; o += up256(4ull * p->n_tiles_stream);
         p->o_chain = o; o += up256(4ull * chain_sync_words((uint32_t)nb));
+        p->lit_q_cap = (uint32_t)(p->total_lit / LONG_LIT);         // every queued piece is longer than LONG_LIT bytes
+        p->o_litq = o; o += up256(16ull * p->lit_q_cap);
         p->o_dst = o; o += up256(4ull * nm);
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
@@ -208,6 +212,7 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.tile_state = reinterpret_cast<unsigned long long*>(s + p->o_tiles);
     P.tile_blk = reinterpret_cast<uint32_t*>(s + p->o_tblk);
     P.chain_sync = reinterpret_cast<uint32_t*>(s + p->o_chain);
+    P.lit_q = reinterpret_cast<uint4*>(s + p->o_litq); P.lit_q_cap = p->lit_q_cap;
     P.wl_dst = reinterpret_cast<uint32_t*>(s + p->o_dst);
     P.wl_off = reinterpret_cast<uint32_t*>(s + p->o_off);
     P.wl_len = reinterpret_cast<uint16_t*>(s + p->o_len);
@@ -236,7 +241,8 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
                 if (ez != cudaSuccess) return ez;
             }
             launch_index(P, st); launch_tilesum(P, p->n_sm * 8, st); launch_pass(P, 0, p->pass_grid, st);
-            n += 2 + (P.n_tiles ? 1 : 0);
+            launch_litcopy(P, p->n_sm * 8, st);
+            n += 2 + (P.n_tiles ? 1 : 0) + (P.lit_q_cap ? 1 : 0);
         }
         if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
             // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
@@ -257,6 +263,7 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
         launch_tilesum(P, p->n_sm * 8, st); ++n;
         if (chain) { launch_pass(P, 0, p->pass_grid, st); n += P.n_tiles ? 1 : 0; }   // literal scatter only: the chain pass validates and counts
         else { launch_pre(P, p->pre_grid, st); n += (P.n_tiles ? 1 : 0) + (P.list_hi ? 1 : 0); }
+        launch_litcopy(P, p->n_sm * 8, st); n += P.lit_q_cap ? 1 : 0;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

@@ -31,6 +31,8 @@ constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in share
 #endif
 constexpr int PERSIST_THREADS = AX_PT;             // k_waves: 1024 threads, one CTA per SM (measured best: DESIGN.md 6.2)
 constexpr uint32_t SHORT_MAX = 32;                 // matches up to this length are copied by one thread
+constexpr uint32_t LONG_LIT = 64;                  // literal runs longer than this are queued and copied by the whole grid (k_litcopy)
+constexpr uint32_t LIT_PIECE = 4096;               // ... in pieces of at most this many bytes
 
 // Per-block descriptor written by k_index (step a1).  Stream addresses are byte offsets from comp base.
 struct BlockDesc {
@@ -45,7 +47,8 @@ struct Status {
     uint32_t fault_block;                          // atomicMin; 0xFFFFFFFF = none
     unsigned long long match_src_bytes;            // M_src counted during PRE
     uint32_t n_final;                              // matches copied by the chain pass (checked against the header)
-    uint32_t pad0[27];
+    uint32_t lit_q_count;                          // long literal runs queued for k_litcopy
+    uint32_t pad0[26];
     uint32_t barrier;                              // grid barrier counter of the persistent wave kernel
     uint32_t pad1[31];
 };
@@ -62,6 +65,8 @@ struct Params {
     unsigned long long* tile_state;                // [n_tiles] exclusive (out << 32 | lit) prefix of the tile inside its block
     uint32_t* tile_blk;                            // [n_tiles] block index of the tile
     uint32_t* chain_sync;                          // strategy CHAIN: [0] frontier, [32 + b] finished tiles of block b
+    uint4* lit_q;                                  // [lit_q_cap] long literal runs: (dst, len, src offset in comp lo, hi)
+    uint32_t lit_q_cap;
     uint32_t* wl_dst;                              // [n_list] match destination (absolute)
     uint32_t* wl_off;                              // [n_list] match source (absolute)
     uint16_t* wl_len;                              // [n_list]
@@ -171,6 +176,35 @@ __device__ __forceinline__ void group_copy(uint8_t* dst, const uint8_t* src, uin
 
 __device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint32_t n, uint32_t lane) {
     group_copy<32>(dst, src, n, lane);
+}
+
+// ---- step a4, long literal runs: a run of more than LONG_LIT bytes is not copied by the thread that parsed it — one warp
+// per run, run after run, leaves the warp waiting on one DRAM round trip per run, and a tile of incompressible data holds
+// up to 2048 x 65 535 literal bytes (one CTA would copy 128 MB while the others idle): measured 7.7 ms of literal scatter
+// on stress2g.  It is queued here, cut into pieces of at most LIT_PIECE bytes, and k_litcopy spreads the queue over the
+// whole grid, one half-warp per piece.  Every piece is longer than LONG_LIT bytes, which bounds the queue by the
+// header's total_lit.
+// Warp-converged call; `has` selects the lanes that queue a run: one atomic per warp reserves the slots of all its lanes.
+__device__ __forceinline__ void queue_long_literals(const Params& P, bool has, uint32_t dst, unsigned long long src_off, uint32_t len, uint32_t lane, uint32_t block) {
+    if (!__any_sync(0xFFFFFFFFu, has)) return;
+    const uint32_t np = has ? (len + LIT_PIECE - 1) / LIT_PIECE : 0u;
+    uint32_t inc = np;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+        if (lane >= (uint32_t)d) inc += t;
+    }
+    uint32_t base = 0;
+    if (lane == 31) base = atomicAdd(&P.status->lit_q_count, inc);
+    base = __shfl_sync(0xFFFFFFFFu, base, 31) + inc - np;
+    if (np) {
+        const uint32_t piece = (len + np - 1) / np;
+        for (uint32_t k = 0, at = 0; k < np; ++k, at += piece) {
+            const uint32_t n = len - at < piece ? len - at : piece;
+            if (base + k < P.lit_q_cap) P.lit_q[base + k] = make_uint4(dst + at, n, (uint32_t)(src_off + at), (uint32_t)((src_off + at) >> 32));
+            else raise_fault(P.status, F_BLOCK_SUM, block);  // more long runs than total_lit allows: the header lied
+        }
+    }
 }
 
 }  // namespace ax

@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
     const uint8_t* hist = dir + (uint64_t)DIR_BYTES * P.n_blocks;
     if (threadIdx.x == 0) {
         P.status->fault_flags = 0; P.status->fault_block = 0xFFFFFFFFu; P.status->match_src_bytes = 0ull;
-        P.status->n_final = 0; P.status->barrier = 0;
+        P.status->n_final = 0; P.status->lit_q_count = 0; P.status->barrier = 0;
     }
     __syncthreads();
     const uint64_t meta = (HDR_BYTES + (uint64_t)DIR_BYTES * P.n_blocks + (uint64_t)HIST_BYTES * (P.max_depth + 1ull) + 127ull) & ~127ull;

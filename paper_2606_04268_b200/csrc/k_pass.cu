@@ -88,8 +88,9 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
         const uint32_t blk_lo = (uint32_t)B.out_base;
         if (LIT) {
             // ---- a4 literal scatter (token validation, M_src and the per-depth counts are taken by the pass that
-            // copies the match: pass 0 reads only cmd[], len[] and lit[]).  Runs of up to 16 bytes: one thread, byte by
-            // byte (the typical run on compressible data is 1-2 bytes); longer runs: the whole warp, 16-byte vector stores.
+            // copies the match: pass 0 reads only cmd[], len[] and lit[]).  Runs of up to LONG_LIT bytes: one thread, byte by
+            // byte (the typical run on compressible data is 1-2 bytes); longer runs: queued for k_litcopy, which spreads
+            // them over the whole grid with 16-byte vector stores.
             const uint8_t* lit = P.comp + B.lit_off;
             uint8_t* outb = P.out + B.out_base;
 #pragma unroll
@@ -98,14 +99,8 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
                 if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
                 const uint32_t cc = ok ? c[k] : 0;
                 if (__any_sync(0xFFFFFFFFu, cc != 0)) {  // literal runs are rare on compressible data: skip as a warp
-                    if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
-                    uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
-                    while (longm) {
-                        const int sl = __ffs(longm) - 1; longm &= longm - 1;
-                        const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, sl), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, sl),
-                                       n2 = __shfl_sync(0xFFFFFFFFu, cc, sl);
-                        warp_copy(outb + p2, lit + s2, n2, lane);
-                    }
+                    if (cc && cc <= LONG_LIT) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
+                    queue_long_literals(P, cc > LONG_LIT, blk_lo + pos, B.lit_off + lsrc, cc, lane, b);       // copied by k_litcopy
                 }
                 pos += c[k] + l[k]; lsrc += c[k];
             }
@@ -174,6 +169,24 @@ int pass_max_ctas_per_sm() {
     int n = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
     return n;
+}
+
+// ---- step a4, the queued pieces of long literal runs: one half-warp per piece (16 lanes x 16 bytes per step), pieces strided
+// over all half-warps of the grid, so that thousands of independent copies are in flight
+constexpr int LC_THREADS = 256;
+__global__ void __launch_bounds__(LC_THREADS) k_litcopy(Params P) {
+    if (P.status->fault_flags & (F_INDEX | F_BLOCK_SUM)) return;
+    uint32_t n = P.status->lit_q_count;
+    if (n > P.lit_q_cap) n = P.lit_q_cap;
+    const uint32_t hw = (blockIdx.x * LC_THREADS + threadIdx.x) >> 4, nhw = (gridDim.x * LC_THREADS) >> 4, l16 = threadIdx.x & 15u;
+    for (uint32_t i = hw; i < n; i += nhw) {
+        const uint4 e = P.lit_q[i];
+        group_copy<16>(P.out + e.x, P.comp + (((unsigned long long)e.w << 32) | e.z), e.y, l16);
+    }
+}
+
+void launch_litcopy(const Params& P, int grid, cudaStream_t st) {
+    if (P.lit_q_cap) k_litcopy<<<grid, LC_THREADS, 0, st>>>(P);
 }
 
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {

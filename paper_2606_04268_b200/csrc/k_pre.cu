@@ -91,14 +91,8 @@ __global__ void __launch_bounds__(PRE_THREADS, 1024 / PRE_THREADS) k_pre(Params 
             if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
             const uint32_t cc = ok ? c[k] : 0;
             if (__any_sync(0xFFFFFFFFu, cc != 0)) {          // literal runs are rare on compressible data: skip as a warp
-                if (cc && cc <= 16) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
-                uint32_t longm = __ballot_sync(0xFFFFFFFFu, cc > 16);
-                while (longm) {                              // long runs by the whole warp
-                    const int src_lane = __ffs(longm) - 1; longm &= longm - 1;
-                    const uint32_t p2 = __shfl_sync(0xFFFFFFFFu, pos, src_lane), s2 = __shfl_sync(0xFFFFFFFFu, lsrc, src_lane),
-                                   n2 = __shfl_sync(0xFFFFFFFFu, cc, src_lane);
-                    warp_copy(outb + p2, lit + s2, n2, lane);
-                }
+                if (cc && cc <= LONG_LIT) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
+                queue_long_literals(P, cc > LONG_LIT, (uint32_t)B.out_base + pos, B.lit_off + lsrc, cc, lane, b);   // copied by k_litcopy
             }
             pos += c[k]; lsrc += c[k];
             bool m = ok && l[k] != 0;
