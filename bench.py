@@ -407,7 +407,8 @@ def measure(name, args, env) -> dict:
               "passes": "k_pass (one streaming pass over the token stream per depth)",
               "persistent": "k_waves (all match waves of one step in one cooperative launch, grid barrier per depth)"}.get(
                   strat, "k_waves (one launch per depth)")
-    tr = ncu_traffic(name) if args.size_mb is None and not args.enc_override else None
+    tr = ncu_traffic(name) if args.size_mb is None and not args.enc_override and args.strategy == "auto" else None
+    b_roof = b_e2e if strat == "chain" else b_match
     rep = {
         "value": round(aggregate_gbs(N, ms_step, world), 2), "ms_per_step": round(ms_step, 4),
         "config": {"workload": name, "raw_bytes": int(N), "comp_bytes": int(C), "n_seq": st["n_seq"], "n_match": nm,
@@ -428,11 +429,15 @@ def measure(name, args, env) -> dict:
         "pre_phase": {"ms": round(ms_pre, 4), "ms_stats": summarize(pre_ms)},
         "waves": {"n_waves": len(waves), "matches_per_wave_min_med_max": [int(min(waves)), int(sorted(waves)[len(waves) // 2]), int(max(waves))] if waves else [],
                   "depth_hist_head": [[d, int(cnt[d]), int(byt[d])] for d in range(min(len(cnt), 9))]},
+        # the match kernel(s) of one step.  Algorithmic bytes: list / pass strategies read 6 B per match + the
+        # sources and write the match bytes (B_match); k_chain reads the whole compressed stream and the sources and writes
+        # the whole output, literal bytes included (B_e2e = C + M_src + N)
         "roofline": {"bound": "hbm", "kernel": kernel,
-                     "achieved": round(gbs(b_match, ms_match), 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-                     "frac": round(gbs(b_match, ms_match) / peak, 4), "traffic": tr["bytes"] if tr else None,
+                     "achieved": round(gbs(b_roof, ms_match), 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                     "frac": round(gbs(b_roof, ms_match) / peak, 4), "traffic": tr["bytes"] if tr else None,
                      "traffic_source": ({"capture": tr["capture"], "commit": tr["commit"]} if tr else None),
-                     "algorithmic_bytes": int(b_match), "kernel_ms": round(ms_match, 4), "share_of_step": round(ms_match / ms_step, 3)},
+                     "algorithmic_bytes": int(b_roof), "algorithmic_bytes_formula": "C + M_src + N" if strat == "chain" else "6*n_match + M_src + M",
+                     "kernel_ms": round(ms_match, 4), "share_of_step": round(ms_match / ms_step, 3)},
         "e2e": {"value": round(world * gbs(N, ms_e2e), 2), "unit": "GB/s", "h2d_bytes_per_step": int(C), "d2h_bytes_per_step": int(N),
                 "two_in_flight": ({"value": round(world * gbs(N, pipe_ms), 2), "unit": "GB/s", "ms": round(pipe_ms, 3),
                                    "note": "two plans on two streams: step i's D2H overlaps step i+1's H2D"} if pipe_ms else pipe_note),
