@@ -6,8 +6,10 @@
  * every match sits at a known dependency depth (PAPER.md:57-63 §3.3, :155 §7.1).  The decoded result is,
  * by definition, what the sequential walk of PAPER.md:53 produces: per block, per sequence, copy the
  * literal run, then copy len bytes from out[off..] in ascending order.  This library reaches exactly
- * that result as: block/token index -> exclusive length scan -> literal scatter -> depth bucketing ->
- * one match-copy wave per dependency depth (§4.4/§7.1).  Byte layout of the
+ * that result as: block/token index -> exclusive length scan -> literal scatter -> match copy in an order
+ * that respects the dependencies: one wave per dependency depth from bucketed lists or by one streaming
+ * pass per depth (§4.4/§7.1), or — for flattened streams — one pass in block order
+ * (after chain flattening a match depends on earlier blocks only).  Byte layout of the
  * compressed buffer: docs/FORMAT.md (version 1).
  *
  * Conventions.  No C++ or PyTorch types.  "host" / "device" is stated per pointer.  All functions
@@ -112,8 +114,9 @@ int aceapex_set_strategy(aceapex_plan_t* p, int strategy);
 
 /* aceapex_decode — enqueue the decode on `stream` and return without synchronising the host.
  *   comp_dev      DEVICE pointer, the same comp_bytes given to aceapex_plan, 16-byte aligned, read only.
- *   out_dev       DEVICE pointer, >= aceapex_out_bytes(p) bytes, 16-byte aligned.  PHASE_PRE first zeroes
- *                 bytes [0, raw) (short matches are OR-merged into zeros), then bytes [0, raw) are written.
+ *   out_dev       DEVICE pointer, >= aceapex_out_bytes(p) bytes, 16-byte aligned.  Under every strategy but CHAIN,
+ *                 PHASE_PRE first zeroes bytes [0, raw) (short matches are OR-merged into zeros); then bytes
+ *                 [0, raw) are written.  Contents on entry do not matter.
  *   scratch_dev   DEVICE pointer, >= aceapex_scratch_bytes(p) bytes, 16-byte aligned.  Contents are
  *                 undefined on entry for PHASE_PRE; PHASE_MATCH alone reuses what PRE left there.
  *   phases        ACEAPEX_PHASE_* mask.  MATCH alone requires a completed PRE on the same scratch and out

@@ -43,6 +43,7 @@ struct aceapex_plan_s {
     uint64_t raw_size, total_seq, total_lit, comp_bytes, n_match;
     std::vector<uint64_t> hist_cnt, hist_bytes;     // [max_depth + 1]
     uint32_t lit_q_cap;                             // capacity of the long-literal queue
+    uint32_t list_mask;                             // strategy PASSES: sparse depths (listed by the literal pass)
     uint32_t n_tiles_list, n_tiles_stream;          // tiles at TILE_LIST / TILE_STREAM sequences per tile
     // device facts
     int device, n_sm, pre_grid, match_ctas_per_sm, chain_grid, pass_grid;
@@ -79,7 +80,8 @@ extern "C" const char* aceapex_strerror(int code) {
 
 // Wave strategy = the cheapest of four cost estimates built from the header (sequences, matches, blocks, depths with
 // matches) and per-unit costs measured on B200 (picoseconds per sequence / match, microseconds per step):
-//   PASSES      literal pass 6.1 ps/seq + per depth one streaming pass 3.6 ps/seq (+ ~3 us launch) + 8.8 ps per match copied
+//   PASSES      literal pass 6.1 ps/seq (7.5 when it lists sparse depths) + per dense depth one streaming pass 3.6 ps/seq
+//               (+ ~3 us launch) + 8.8 ps per match copied; per sparse depth one list wave (5.5 us + 21 ps per match)
 //   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5.5 us + 21 ps per match copied from a list
 //   PERSISTENT  the same lists, one cooperative kernel: ~4 us of grid barrier + fence drain + straggler wait per depth
 //   CHAIN       (FLATTENED streams only) literal pass 3.1 ps/seq, then one pass whose time is the larger of the block chain
@@ -92,7 +94,12 @@ static int choose_strategy(const aceapex_plan_t* p) {
     const double seq = (double)p->total_seq, m = (double)p->n_match;
     const double t_lists = 14.5e-6 * seq + 21e-6 * m;                           // microseconds
     const double t_launch = t_lists + 5.5 * waves, t_persist = t_lists + 4.0 * waves + 8.0;
-    const double t_passes = p->max_depth <= PASS_MAX_DEPTH ? 6.1e-6 * seq + p->max_depth * (3.6e-6 * seq + 3.0) + 8.8e-6 * m : 1e300;
+    double t_passes = 1e300;
+    if (p->max_depth <= PASS_MAX_DEPTH) {
+        t_passes = (p->list_mask ? 7.5e-6 : 6.1e-6) * seq;                     // literal pass (+ listing the sparse depths)
+        for (uint32_t d = 1; d <= p->max_depth; ++d)
+            t_passes += ((p->list_mask >> d) & 1u) ? 5.5 + 21e-6 * (double)p->hist_cnt[d] : 3.0 + 3.6e-6 * seq + 8.8e-6 * (double)p->hist_cnt[d];
+    }
     const double hop = 6.5 * p->n_blocks, thr = 26e-6 * seq;
     const double t_chain = (p->flags & FLAG_FLATTENED) ? 3.1e-6 * seq + (hop > thr ? hop : thr) + 10.0 : 1e300;
     int best = ACEAPEX_WAVES_LAUNCH; double t = t_launch;
@@ -179,6 +186,12 @@ extern "C" int aceapex_plan(const void* comp_host, size_t comp_bytes, int device
         p->o_off = o; o += up256(4ull * nm);
         p->o_len = o; o += up256(2ull * nm);
         p->scratch_bytes = o;
+        // strategy PASSES: a depth holding fewer than 1/8 of the sequences is cheaper to list in the literal pass and copy
+        // from the list (21 ps per match) than to find with a sweep over the whole stream (3.6 ps per sequence)
+        p->list_mask = 0;
+        if (p->max_depth <= PASS_MAX_DEPTH)
+            for (uint32_t d = 1; d <= p->max_depth; ++d)
+                if (p->hist_cnt[d] && p->hist_cnt[d] * 8 < p->total_seq) p->list_mask |= 1u << d;
         p->strategy_forced = ACEAPEX_WAVES_AUTO;
         p->strategy_auto = choose_strategy(p);
         p->last_strategy = p->strategy_auto;
@@ -221,6 +234,7 @@ static Params make_params(const aceapex_plan_t* p, const void* comp_dev, void* o
     P.tile = stream_tiles ? TILE_STREAM : TILE_LIST; P.n_tiles = stream_tiles ? p->n_tiles_stream : p->n_tiles_list; P.max_depth = p->max_depth; P.min_match = p->min_match;
     // strategy CHAIN: no wave list at all (k_chain copies every match straight from the stream, in block order)
     P.list_hi = strategy == ACEAPEX_WAVES_CHAIN ? 0 : p->max_depth;
+    P.list_mask = strategy == ACEAPEX_WAVES_PASSES ? p->list_mask : 0;
     uint64_t nl = 0;
     for (uint32_t d = 1; d <= P.list_hi; ++d) nl += p->hist_cnt[d];
     P.n_list = (uint32_t)nl;
@@ -246,8 +260,15 @@ static cudaError_t enqueue(aceapex_plan_t* p, const Params& P, unsigned phases, 
         }
         if ((phases & ACEAPEX_PHASE_MATCH) && p->max_depth) {
             // every depth gets its pass, also one the histogram calls empty: the passes do the token validation
+            // (a sparse depth was listed by the literal pass: its matches are copied from the list)
             launch_pass_reset(P, st); ++n;
-            for (uint32_t d = 1; d <= p->max_depth; ++d) { launch_pass(P, d, p->pass_grid, st); n += P.n_tiles ? 1 : 0; }
+            for (uint32_t d = 1; d <= p->max_depth; ++d) {
+                if ((P.list_mask >> d) & 1u) {
+                    cudaError_t e = launch_wave(P, d, (uint32_t)p->hist_cnt[d], p->n_sm * p->match_ctas_per_sm, st);
+                    if (e != cudaSuccess) return e;
+                    ++n;
+                } else { launch_pass(P, d, p->pass_grid, st); n += P.n_tiles ? 1 : 0; }
+            }
             launch_check_cursors(P, st); ++n;
         }
         *n_launch = n;
@@ -382,7 +403,7 @@ extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, ace
         cudaError_t e = cudaStreamSynchronize(p->last_stream);
         if (e == cudaSuccess) e = cudaMemcpy(&h, static_cast<const uint8_t*>(scratch_dev) + p->o_status, sizeof h, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
-        s->match_src_bytes = h.match_src_bytes; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
+        s->match_src_bytes = h.match_src_bytes + h.src_bytes_pre; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
         // strategy SPAN keeps no list (hence no cursor) for the last depth: its count comes back from the span pass
         // strategy CHAIN keeps no list (hence no cursor): its match count comes back from the chain pass
         if (!h.fault_flags && p->last_strategy == ACEAPEX_WAVES_CHAIN && p->max_depth && p->last_had_match && h.n_final != p->n_match) {

@@ -48,7 +48,8 @@ struct Status {
     unsigned long long match_src_bytes;            // M_src counted during PRE
     uint32_t n_final;                              // matches copied by the chain pass (checked against the header)
     uint32_t lit_q_count;                          // long literal runs queued for k_litcopy
-    uint32_t pad0[26];
+    unsigned long long src_bytes_pre;              // M_src of the matches listed by the literal pass (strategy PASSES, sparse depths)
+    uint32_t pad0[24];
     uint32_t barrier;                              // grid barrier counter of the persistent wave kernel
     uint32_t pad1[31];
 };
@@ -74,6 +75,8 @@ struct Params {
     uint32_t block_size, n_blocks, n_tiles, tile, max_depth, min_match;   // tile: sequences per tile (TILE_LIST or TILE_STREAM)
     uint32_t n_list;                               // capacity of the wave lists = matches at depths 1 .. list_hi
     uint32_t list_hi;                              // depths 1 .. list_hi travel through wave lists (0: strategy CHAIN, no lists)
+    uint32_t list_mask;                            // strategy PASSES: bit d set = depth d is sparse: the literal pass lists its
+                                                   // matches and a list wave copies them; the other depths get a streaming pass
 };
 
 __host__ __device__ inline uint64_t pad16(uint64_t x) { return (x + 15) & ~(uint64_t)15; }

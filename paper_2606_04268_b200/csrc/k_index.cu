@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(IDX_THREADS) k_index(Params P) {
     const uint8_t* dir = P.comp + HDR_BYTES;
     const uint8_t* hist = dir + (uint64_t)DIR_BYTES * P.n_blocks;
     if (threadIdx.x == 0) {
-        P.status->fault_flags = 0; P.status->fault_block = 0xFFFFFFFFu; P.status->match_src_bytes = 0ull;
+        P.status->fault_flags = 0; P.status->fault_block = 0xFFFFFFFFu; P.status->match_src_bytes = 0ull; P.status->src_bytes_pre = 0ull;
         P.status->n_final = 0; P.status->lit_q_count = 0; P.status->barrier = 0;
     }
     __syncthreads();

@@ -20,13 +20,14 @@ constexpr int PS_WCAP = 32 * PRE_ITEMS;                  // matches one warp can
 struct PassSmem {
     unsigned long long warp_sum[PS_WARPS];
     uint32_t cnt;                                        // matches this CTA copied in this pass (histogram check)
+    uint32_t lcnt[PASS_MAX_DEPTH + 1], lbase[PASS_MAX_DEPTH + 1];   // literal pass: the tile's listed matches per sparse depth, their list slots
     uint32_t w_dst[PS_WARPS][PS_WCAP];                   // per warp: the tile's matches of this pass, compacted
     uint32_t w_off[PS_WARPS][PS_WCAP];
     uint16_t w_len[PS_WARPS][PS_WCAP];
 };
 
-// ---- pass p: 0 = literals, p >= 1 = matches of depth p
-template <bool LIT>
+// ---- pass p: 0 = literals (LISTING: and the wave lists of the sparse depths), p >= 1 = matches of depth p
+template <bool LIT, bool LISTING>
 __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P, uint32_t p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PassSmem& S = *reinterpret_cast<PassSmem*>(smem_raw);
@@ -35,6 +36,8 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
     if (P.status->fault_flags & F_INDEX) return;                    // the block index is inconsistent (k_index): touch nothing
     if (!LIT && P.status->fault_flags != 0) return;                 // a faulty stream is flagged, not decoded further
     if (tid == 0) S.cnt = 0;
+    constexpr bool listing = LIT && LISTING;                        // some depths are sparse: their matches are listed here
+    if (listing && tid <= PASS_MAX_DEPTH) S.lcnt[tid] = 0;
     __syncthreads();
     for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         const uint32_t b = P.tile_blk[tile];
@@ -43,7 +46,7 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
         const uint32_t j0 = (tile - B.tile_base) * TILE_STREAM + tid * PRE_ITEMS;
         // ---- a2: parse (pass 0 needs neither depths nor sources)
         Seq8 q;
-        load_seq8(q, P.comp, B, j0, !LIT);
+        load_seq8(q, P.comp, B, j0, !LIT || listing);
         uint32_t (&c)[PRE_ITEMS] = q.c, (&l)[PRE_ITEMS] = q.l, (&dp)[PRE_ITEMS] = q.dp, (&of)[PRE_ITEMS] = q.of;
         // ---- a3: scan inside the tile; the block-level prefix comes from k_tilesum.  The literal pass scans the pair
         // (cmd+len, cmd) packed in one u64; match passes need output positions only (32-bit shuffles)
@@ -93,9 +96,21 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
             // them over the whole grid with 16-byte vector stores.
             const uint8_t* lit = P.comp + B.lit_off;
             uint8_t* outb = P.out + B.out_base;
+            const uint32_t pos0 = pos;
+            uint32_t rank[PRE_ITEMS], sel_mask = 0;                  // (listing) rank of a listed match among its depth's in the tile
 #pragma unroll
             for (int k = 0; k < PRE_ITEMS; ++k) {
                 const bool ok = (uint64_t)pos + c[k] + l[k] <= B.raw_len && (uint64_t)lsrc + c[k] <= B.n_lit;
+                rank[k] = 0;
+                if (listing && ok && l[k] != 0 && dp[k] <= PASS_MAX_DEPTH && ((P.list_mask >> dp[k]) & 1u)) {
+                    const uint32_t mdst = blk_lo + pos + c[k];
+                    if (of[k] >= mdst || l[k] < P.min_match) raise_fault(P.status, F_SOURCE, b);              // I2
+                    else {
+                        const uint32_t dist = mdst - of[k];
+                        src_bytes += l[k] < dist ? l[k] : dist;
+                        rank[k] = atomicAdd(&S.lcnt[dp[k]], 1u); sel_mask |= 1u << k;
+                    }
+                }
                 if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
                 const uint32_t cc = ok ? c[k] : 0;
                 if (__any_sync(0xFFFFFFFFu, cc != 0)) {  // literal runs are rare on compressible data: skip as a warp
@@ -103,6 +118,25 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
                     queue_long_literals(P, cc > LONG_LIT, blk_lo + pos, B.lit_off + lsrc, cc, lane, b);       // copied by k_litcopy
                 }
                 pos += c[k] + l[k]; lsrc += c[k];
+            }
+            if (listing) {
+                // a5 for the sparse depths only: reserve the tile's slice of each depth's wave list, write the entries
+                __syncthreads();
+                if (tid <= PASS_MAX_DEPTH && S.lcnt[tid]) S.lbase[tid] = atomicAdd(&P.cursor[tid], S.lcnt[tid]);
+                __syncthreads();
+                uint32_t p2 = pos0;
+#pragma unroll
+                for (int k = 0; k < PRE_ITEMS; ++k) {
+                    p2 += c[k];
+                    if (sel_mask & (1u << k)) {
+                        const uint32_t g = S.lbase[dp[k]] + rank[k];
+                        if (g < P.wave_off[dp[k] + 1]) { P.wl_dst[g] = blk_lo + p2; P.wl_off[g] = of[k]; P.wl_len[g] = (uint16_t)l[k]; }
+                        else raise_fault(P.status, F_DEPTH, b);      // more matches than the histogram says
+                    }
+                    p2 += l[k];
+                }
+                __syncthreads();
+                if (tid <= PASS_MAX_DEPTH) S.lcnt[tid] = 0;          // (ordered before the next tile's counting by its scan barriers)
             }
         } else {
             // ---- a6: select this pass's matches (same validity rule as pass 0), compact them per warp, copy
@@ -141,9 +175,11 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
     if (!LIT) {
         __syncthreads();
         if (tid == 0 && S.cnt) atomicAdd(&P.cursor[p], S.cnt);      // histogram check (k_check_cursors after the last pass)
+    }
+    if (!LIT || listing) {
 #pragma unroll
         for (int d = 16; d; d >>= 1) src_bytes += __shfl_xor_sync(0xFFFFFFFFu, src_bytes, d);
-        if (lane == 0 && src_bytes) atomicAdd(&P.status->match_src_bytes, src_bytes);
+        if (lane == 0 && src_bytes) atomicAdd(LIT ? &P.status->src_bytes_pre : &P.status->match_src_bytes, src_bytes);
     }
 }
 
@@ -152,7 +188,7 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
 __global__ void k_pass_reset(Params P) {
     const uint32_t d = blockIdx.x * blockDim.x + threadIdx.x;
     if (d == 0) P.status->match_src_bytes = 0ull;
-    if (d >= 1 && d <= P.max_depth) P.cursor[d] = P.wave_off[d];
+    if (d >= 1 && d <= P.max_depth && !((P.list_mask >> d) & 1u)) P.cursor[d] = P.wave_off[d];   // (listed depths were counted by PRE)
 }
 
 void launch_pass_reset(const Params& P, cudaStream_t st) {
@@ -160,14 +196,15 @@ void launch_pass_reset(const Params& P, cudaStream_t st) {
 }
 
 cudaError_t pass_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    cudaError_t e = cudaFuncSetAttribute(k_pass<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    return e;
 }
 
 int pass_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false, false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
     return n;
 }
 
@@ -192,8 +229,9 @@ void launch_litcopy(const Params& P, int grid, cudaStream_t st) {
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {
     if (!P.n_tiles) return;
     const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
-    if (p == 0) k_pass<true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
-    else k_pass<false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    if (p == 0 && P.list_mask) k_pass<true, true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else if (p == 0) k_pass<true, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else k_pass<false, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
 }
 
 }  // namespace ax
