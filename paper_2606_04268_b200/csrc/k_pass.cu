@@ -1,13 +1,19 @@
 // k_pass.cu — strategy PASSES for shallow streams (e.g. the depth-limited encoder of PAPER.md:228 §7.4, "at most D
-// match waves"): no wave lists at all.  The token stream is parsed once per pass instead:
-//   k_pass 0    parse cmd[], len[] (a2) + scan inside the tile (a3) + literal scatter (a4).
-//   k_pass p    parse + scan + validation (I2), M_src and copy of the matches with dep == p (a6), p = 1 .. max_depth,
-//               one launch each (a7: a kernel boundary orders wave p-1 before wave p); a match whose
-//               dep is 0 or above max_depth is copied by no pass and shows up as a histogram mismatch (F_DEPTH).
-// Why: with few waves the wave lists cost more than they save — 10 B written + 10 B read per match
-// and a bucketing kernel (k_pre) that ranks, reserves and scatters every match — whereas re-reading the 10 B/sequence
-// stream is a pure streaming read with no inter-CTA dependency: tiles are assigned statically, their prefixes inside the
-// block come from k_tilesum, nothing is reserved with atomics.
+// match waves"): the token stream is parsed once per pass instead of being bucketed into wave lists:
+//   k_pass 0    parse cmd[], len[] (a2) + scan inside the tile (a3) + literal scatter (a4).  Instance LISTING: also
+//               reads dep[] / off[] and writes the wave lists of the SPARSE depths (Params::list_mask: depths holding
+//               fewer than 1/8 of the sequences) — validation (I2), M_src, per-depth rank in shared memory, one global
+//               atomic per depth and tile to reserve the tile's slice of the list (a5 for those depths only).
+//   k_pass p    parse + scan + validation (I2), M_src and copy of the matches with dep == p (a6), one launch per DENSE
+//               depth (a7: a kernel boundary orders wave p-1 before wave p); sparse depths are copied from
+//               their lists by k_waves (k_match.cu), in depth order with the passes.  A match whose dep is 0 or above
+//               max_depth is copied by nothing and shows up as a histogram mismatch (F_DEPTH).
+//   k_litcopy   the queued long literal runs (a4), one half-warp per piece, over the whole grid.
+// Why: with few waves, lists for everything cost more than they save — 10 B written + 10 B read per
+// match and a bucketing kernel (k_pre) that ranks, reserves and scatters every match — whereas re-reading the
+// 10 B/sequence stream is a pure streaming read with no inter-CTA dependency: tiles are assigned statically, their
+// prefixes inside the block come from k_tilesum.  A sweep costs ~0.65 ms per 176 M sequences before it copies a byte,
+// so it pays only for a depth that holds many matches; hence the lists for the sparse ones.
 // Matches are copied exactly as in the wave kernel (copy.cuh: register funnel shift, OR-merge into the zeroed output).
 #include "common.cuh"
 #include "copy.cuh"
