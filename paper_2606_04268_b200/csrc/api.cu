@@ -404,7 +404,6 @@ extern "C" int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, ace
         if (e == cudaSuccess) e = cudaMemcpy(&h, static_cast<const uint8_t*>(scratch_dev) + p->o_status, sizeof h, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
         s->match_src_bytes = h.match_src_bytes + h.src_bytes_pre; s->fault_flags = h.fault_flags; s->fault_block = h.fault_block;
-        // strategy SPAN keeps no list (hence no cursor) for the last depth: its count comes back from the span pass
         // strategy CHAIN keeps no list (hence no cursor): its match count comes back from the chain pass
         if (!h.fault_flags && p->last_strategy == ACEAPEX_WAVES_CHAIN && p->max_depth && p->last_had_match && h.n_final != p->n_match) {
             s->fault_flags = F_DEPTH; s->fault_block = 0xFFFFFFFEu;

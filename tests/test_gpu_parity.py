@@ -135,7 +135,10 @@ CASES = [("markov", 1 << 20, dict(block_size=1 << 18)),
          ("fastq", (3 << 20) + 77, dict()),
          ("stress", 6 << 20, dict()),
          ("stress", 4 << 20, dict(flatten=False)),
-         ("stress", 4 << 20, dict(depth_limit=1))]
+         ("stress", 4 << 20, dict(depth_limit=1)),
+         ("text", 3 << 20, dict(min_match=11)),                                          # token-cost-aware regime (Q4):
+         ("fastq", (3 << 20) + 5, dict(min_match=11, depth_limit=4)),                    # long literal runs, fewer and longer matches
+         ("fastq", 2 << 20, dict(min_match=11, max_chain=4, flatten=False))]
 
 
 @pytest.mark.parametrize("kind,n,kw", CASES)
