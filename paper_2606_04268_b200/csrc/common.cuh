@@ -31,7 +31,7 @@ constexpr uint32_t SMEM_DEPTHS = 4096;             // depth bins ranked in share
 #endif
 constexpr int PERSIST_THREADS = AX_PT;             // k_waves: 1024 threads, one CTA per SM (measured best: DESIGN.md 6.2)
 constexpr uint32_t SHORT_MAX = 32;                 // matches up to this length are copied by one thread
-constexpr uint32_t LONG_LIT = 64;                  // literal runs longer than this are queued and copied by the whole grid (k_litcopy)
+constexpr uint32_t LONG_LIT = 16;                  // literal runs longer than this are queued and copied by the whole grid (k_litcopy)
 constexpr uint32_t LIT_PIECE = 4096;               // ... in pieces of at most this many bytes
 
 // Per-block descriptor written by k_index (step a1).  Stream addresses are byte offsets from comp base.
@@ -185,7 +185,7 @@ __device__ __forceinline__ void warp_copy(uint8_t* dst, const uint8_t* src, uint
 // per run, run after run, leaves the warp waiting on one DRAM round trip per run, and a tile of incompressible data holds
 // up to 2048 x 65 535 literal bytes (one CTA would copy 128 MB while the others idle): measured 7.7 ms of literal scatter
 // on stress2g.  It is queued here, cut into pieces of at most LIT_PIECE bytes, and k_litcopy spreads the queue over the
-// whole grid, one half-warp per piece.  Every piece is longer than LONG_LIT bytes, which bounds the queue by the
+// whole grid, eight lanes per piece.  Every piece is longer than LONG_LIT bytes, which bounds the queue by the
 // header's total_lit.
 // Warp-converged call; `has` selects the lanes that queue a run: one atomic per warp reserves the slots of all its lanes.
 __device__ __forceinline__ void queue_long_literals(const Params& P, bool has, uint32_t dst, unsigned long long src_off, uint32_t len, uint32_t lane, uint32_t block) {

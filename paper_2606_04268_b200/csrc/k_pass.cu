@@ -8,7 +8,7 @@
 //               depth (a7: a kernel boundary orders wave p-1 before wave p); sparse depths are copied from
 //               their lists by k_waves (k_match.cu), in depth order with the passes.  A match whose dep is 0 or above
 //               max_depth is copied by nothing and shows up as a histogram mismatch (F_DEPTH).
-//   k_litcopy   the queued long literal runs (a4), one half-warp per piece, over the whole grid.
+//   k_litcopy   the queued long literal runs (a4), eight lanes per piece, over the whole grid.
 // Why: with few waves, lists for everything cost more than they save — 10 B written + 10 B read per
 // match and a bucketing kernel (k_pre) that ranks, reserves and scatters every match — whereas re-reading the
 // 10 B/sequence stream is a pure streaming read with no inter-CTA dependency: tiles are assigned statically, their
@@ -214,17 +214,18 @@ int pass_max_ctas_per_sm() {
     return n;
 }
 
-// ---- step a4, the queued pieces of long literal runs: one half-warp per piece (16 lanes x 16 bytes per step), pieces strided
-// over all half-warps of the grid, so that thousands of independent copies are in flight
+// ---- step a4, the queued pieces of long literal runs: eight lanes per piece (x 16 bytes per step), pieces strided over all
+// lane groups of the grid, so that thousands of independent copies are in flight
 constexpr int LC_THREADS = 256;
 __global__ void __launch_bounds__(LC_THREADS) k_litcopy(Params P) {
     if (P.status->fault_flags & (F_INDEX | F_BLOCK_SUM)) return;
     uint32_t n = P.status->lit_q_count;
     if (n > P.lit_q_cap) n = P.lit_q_cap;
-    const uint32_t hw = (blockIdx.x * LC_THREADS + threadIdx.x) >> 4, nhw = (gridDim.x * LC_THREADS) >> 4, l16 = threadIdx.x & 15u;
+    constexpr uint32_t G = 8;                       // lanes per piece (x 16 bytes per step): 8 / 16 measured on runs of ~260 B
+    const uint32_t hw = (blockIdx.x * LC_THREADS + threadIdx.x) / G, nhw = (gridDim.x * LC_THREADS) / G, l16 = threadIdx.x % G;
     for (uint32_t i = hw; i < n; i += nhw) {
         const uint4 e = P.lit_q[i];
-        group_copy<16>(P.out + e.x, P.comp + (((unsigned long long)e.w << 32) | e.z), e.y, l16);
+        group_copy<G>(P.out + e.x, P.comp + (((unsigned long long)e.w << 32) | e.z), e.y, l16);
     }
 }
 
