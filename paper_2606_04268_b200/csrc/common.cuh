@@ -68,6 +68,7 @@ struct Params {
     uint32_t* chain_sync;                          // strategy CHAIN: [0] frontier, [32 + b] finished tiles of block b
     uint4* lit_q;                                  // [lit_q_cap] long literal runs: (dst, len, src offset in comp lo, hi)
     uint32_t lit_q_cap;
+    uint32_t long_runs;                            // the header's mean literal run is 4-20 bytes (picks the literal pass instance)
     uint32_t* wl_dst;                              // [n_list] match destination (absolute)
     uint32_t* wl_off;                              // [n_list] match source (absolute)
     uint16_t* wl_len;                              // [n_list]

@@ -33,7 +33,7 @@ struct PassSmem {
 };
 
 // ---- pass p: 0 = literals (LISTING: and the wave lists of the sparse depths), p >= 1 = matches of depth p
-template <bool LIT, bool LISTING>
+template <bool LIT, bool LISTING, bool VECLIT>
 __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P, uint32_t p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PassSmem& S = *reinterpret_cast<PassSmem*>(smem_raw);
@@ -120,7 +120,8 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
                 if (!ok && (c[k] | l[k])) raise_fault(P.status, F_BLOCK_SUM, b);
                 const uint32_t cc = ok ? c[k] : 0;
                 if (__any_sync(0xFFFFFFFFu, cc != 0)) {  // literal runs are rare on compressible data: skip as a warp
-                    if (cc && cc <= LONG_LIT) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
+                    if (VECLIT && cc > 4 && cc <= LONG_LIT) store16(outb + pos, load16(lit + lsrc, cc), cc);   // (streams of longer runs)
+                    else if (cc && cc <= LONG_LIT) { for (uint32_t i = 0; i < cc; ++i) outb[pos + i] = lit[lsrc + i]; }   // typical run: 1-2 bytes
                     queue_long_literals(P, cc > LONG_LIT, blk_lo + pos, B.lit_off + lsrc, cc, lane, b);       // copied by k_litcopy
                 }
                 pos += c[k] + l[k]; lsrc += c[k];
@@ -202,15 +203,18 @@ void launch_pass_reset(const Params& P, cudaStream_t st) {
 }
 
 cudaError_t pass_configure() {
-    cudaError_t e = cudaFuncSetAttribute(k_pass<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(PassSmem));
+    const int n = (int)sizeof(PassSmem);
+    cudaError_t e = cudaFuncSetAttribute(k_pass<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, n);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, n);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, n);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, n);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_pass<true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, n);
     return e;
 }
 
 int pass_max_ctas_per_sm() {
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false, false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_pass<false, false, false>, PS_THREADS, sizeof(PassSmem)) != cudaSuccess) return 0;
     return n;
 }
 
@@ -236,9 +240,14 @@ void launch_litcopy(const Params& P, int grid, cudaStream_t st) {
 void launch_pass(const Params& P, uint32_t p, int grid, cudaStream_t st) {
     if (!P.n_tiles) return;
     const uint32_t g = (uint32_t)grid < P.n_tiles ? grid : P.n_tiles;
-    if (p == 0 && P.list_mask) k_pass<true, true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
-    else if (p == 0) k_pass<true, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
-    else k_pass<false, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    // Literal pass: the instance is picked from the header — with sparse depths it also lists them; where the mean literal run
+    // is 4-20 bytes, runs of 5-16 bytes go through one 16-byte register value instead of the byte loop (separate instances,
+    // so that the common one — runs of 1-2 bytes — keeps its short unrolled token loop: DESIGN.md 6.7).
+    if (p == 0 && P.list_mask && P.long_runs) k_pass<true, true, true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else if (p == 0 && P.list_mask) k_pass<true, true, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else if (p == 0 && P.long_runs) k_pass<true, false, true><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else if (p == 0) k_pass<true, false, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
+    else k_pass<false, false, false><<<g, PS_THREADS, sizeof(PassSmem), st>>>(P, p);
 }
 
 }  // namespace ax
