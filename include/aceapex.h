@@ -40,7 +40,8 @@ enum {
     ACEAPEX_E_CUDA = -7,      /* a CUDA runtime call failed (see aceapex_last_cuda_error)             */
     ACEAPEX_E_ARG = -8,       /* NULL / out-of-range argument                                         */
     ACEAPEX_E_STREAM = -9,    /* token-level fault found on the device (see aceapex_stats.fault_*)    */
-    ACEAPEX_E_NOMEM = -10     /* host allocation failed                                               */
+    ACEAPEX_E_NOMEM = -10,    /* host allocation failed                                               */
+    ACEAPEX_E_NOALLOC_LIMIT = -11 /* aceapex_decode_noalloc: the stream needs more scratch than the static buffer holds */
 };
 
 /* phases bitmask of aceapex_decode */
@@ -153,6 +154,20 @@ int aceapex_get_stats(aceapex_plan_t* p, const void* scratch_dev, aceapex_stats*
  * number of matches / match bytes at depth d (d = 0: literal runs / literal bytes).  Returns the number
  * of entries available (max_depth + 1) or a negative error. */
 int64_t aceapex_depth_hist(const aceapex_plan_t* p, uint64_t* n_match, uint64_t* n_bytes, uint32_t cap);
+
+/* aceapex_decode_noalloc — the full decode (PHASE_ALL) for callers that cannot provide device scratch and must not
+ * trigger an allocation (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same
+ * kernels, same comp_dev / out_dev / stream meaning as aceapex_decode; the scratch is ONE static device array owned by
+ * the library: aceapex_noalloc_max_scratch_bytes() = 16 MiB, held by every GPU that loads the library until the process
+ * exits.  A plan whose aceapex_scratch_bytes exceeds that is rejected with ACEAPEX_E_NOALLOC_LIMIT (nothing is launched).
+ * The call performs no cudaMalloc / cudaFree / allocating library routine (strategy GRAPH is run as LAUNCH).  Every call
+ * on a device shares the array and finds the last call's contents in it; nothing relies on them (the pre-phase resets what
+ * must start at zero).  Calls that overlap on the GPU — two streams, two plans, two threads — RACE on the array: one decode
+ * at a time per device, and aceapex_get_stats_noalloc (same meaning as aceapex_get_stats) before the next one.
+ * Errors: E_ARG (also: current device is not the plan's), E_NOALLOC_LIMIT, E_CAPACITY, E_ALIGN, E_CUDA. */
+int aceapex_decode_noalloc(aceapex_plan_t* p, const void* comp_dev, void* out_dev, size_t out_capacity, void* stream);
+int aceapex_get_stats_noalloc(aceapex_plan_t* p, aceapex_stats* s);
+size_t aceapex_noalloc_max_scratch_bytes(void);
 
 const char* aceapex_strerror(int code);
 int aceapex_last_cuda_error(const aceapex_plan_t* p); /* cudaError_t of the last failing CUDA call, else 0 */

@@ -17,7 +17,7 @@ _SOURCES = ["k_index.cu", "k_tilesum.cu", "k_pre.cu", "k_match.cu", "k_pass.cu",
 _HEADERS = [os.path.join(_CSRC, "common.cuh"), os.path.join(_CSRC, "copy.cuh"), os.path.join(os.path.dirname(_HERE), "include", "aceapex.h")]
 
 OK = 0
-E_MAGIC, E_VERSION, E_TRUNCATED, E_HEADER, E_CAPACITY, E_ALIGN, E_CUDA, E_ARG, E_STREAM, E_NOMEM = range(-1, -11, -1)
+E_MAGIC, E_VERSION, E_TRUNCATED, E_HEADER, E_CAPACITY, E_ALIGN, E_CUDA, E_ARG, E_STREAM, E_NOMEM, E_NOALLOC_LIMIT = range(-1, -12, -1)
 PHASE_PRE, PHASE_MATCH, PHASE_ALL = 1, 2, 3
 WAVES_AUTO, WAVES_LAUNCH, WAVES_GRAPH, WAVES_PERSISTENT, WAVES_PASSES, WAVES_CHAIN = 0, 1, 2, 3, 4, 5
 STRATEGY_NAMES = {0: "auto", 1: "launch", 2: "graph", 3: "persistent", 4: "passes", 5: "chain"}
@@ -25,7 +25,8 @@ F_BLOCK_SUM, F_SOURCE, F_DEPTH, F_PLACEHOLDER, F_INDEX = 1, 2, 4, 8, 16
 
 EXPORTS = ["aceapex_plan", "aceapex_raw_bytes", "aceapex_out_bytes", "aceapex_scratch_bytes", "aceapex_set_strategy",
            "aceapex_decode", "aceapex_decode_host", "aceapex_get_stats", "aceapex_depth_hist", "aceapex_strerror",
-           "aceapex_last_cuda_error", "aceapex_free"]
+           "aceapex_last_cuda_error", "aceapex_free", "aceapex_decode_noalloc", "aceapex_get_stats_noalloc",
+           "aceapex_noalloc_max_scratch_bytes"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -82,6 +83,9 @@ def _lib():
         L.aceapex_strerror.argtypes = [ctypes.c_int]; L.aceapex_strerror.restype = ctypes.c_char_p
         L.aceapex_last_cuda_error.argtypes = [vp]; L.aceapex_last_cuda_error.restype = ctypes.c_int
         L.aceapex_free.argtypes = [vp]; L.aceapex_free.restype = None
+        L.aceapex_decode_noalloc.argtypes = [vp, vp, vp, sz, vp]; L.aceapex_decode_noalloc.restype = ctypes.c_int
+        L.aceapex_get_stats_noalloc.argtypes = [vp, ctypes.POINTER(Stats)]; L.aceapex_get_stats_noalloc.restype = ctypes.c_int
+        L.aceapex_noalloc_max_scratch_bytes.argtypes = []; L.aceapex_noalloc_max_scratch_bytes.restype = sz
         _LIB = L
     return _LIB
 
@@ -124,6 +128,20 @@ class Plan:
                     out_dev: int, out_capacity: int, scratch_dev: int, scratch_bytes: int, stream: int = 0):
         _check(self._L.aceapex_decode_host(self._h, comp_host, comp_bytes, out_host, out_host_capacity, comp_dev, out_dev,
                                            out_capacity, scratch_dev, scratch_bytes, stream), "decode_host")
+
+    def decode_noalloc(self, comp_dev: int, out_dev: int, out_capacity: int, stream: int = 0):
+        """aceapex_decode_noalloc: full decode with the library's static device scratch (no allocation; one call at a time)."""
+        rc = self._L.aceapex_decode_noalloc(self._h, comp_dev, out_dev, out_capacity, stream)
+        _check(rc, "decode_noalloc" if rc != E_CUDA else f"decode_noalloc (cudaError {self._L.aceapex_last_cuda_error(self._h)})")
+
+    def stats_noalloc(self, check: bool = True) -> dict:
+        s = Stats()
+        rc = self._L.aceapex_get_stats_noalloc(self._h, ctypes.byref(s))
+        if rc != 0 and (check or rc != E_STREAM):
+            raise AceapexError(rc, "get_stats_noalloc")
+        d = s.as_dict()
+        d["rc"] = rc
+        return d
 
     def stats(self, scratch_dev: int = 0, check: bool = True) -> dict:
         s = Stats()

@@ -5,6 +5,7 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -74,6 +75,7 @@ extern "C" const char* aceapex_strerror(int code) {
         case ACEAPEX_E_ARG: return "bad argument";
         case ACEAPEX_E_STREAM: return "token stream fault detected on the device";
         case ACEAPEX_E_NOMEM: return "host allocation failed";
+        case ACEAPEX_E_NOALLOC_LIMIT: return "stream needs more scratch than the library's static no-allocation buffer holds (aceapex_noalloc_max_scratch_bytes)";
         default: return "unknown error";
     }
 }
@@ -431,4 +433,81 @@ extern "C" void aceapex_free(aceapex_plan_t* p) {
     for (GraphSlot& g : p->graphs) cudaGraphExecDestroy(g.exec);
     if (p->capture_stream) cudaStreamDestroy(p->capture_stream);
     delete p;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// No-allocation entry point (include/aceapex.h: aceapex_decode_noalloc).  For callers that cannot obtain device scratch
+// (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the same kernels, with their
+// scratch (status words, block descriptors, tile prefixes, wave lists, literal queue, chain counters — the layout of
+// aceapex_scratch_bytes) placed in ONE file-scope device array owned by the library.  NOALLOC_MAX bytes are held by every
+// GPU that loads the library, until the process exits.  Nothing here calls cudaMalloc / cudaFree / an allocating routine
+// (strategy GRAPH, which instantiates a graph, is run as LAUNCH).
+//  * In host code the array's NAME is a host-side stand-in, not a device address: the address comes from
+//    cudaGetSymbolAddress, once per device, with that device current (noalloc_scratch below), and that pointer is what the
+//    kernels get (through Params, like a caller's scratch).
+//  * Every call shares the array and finds the previous call's contents in it.  Nothing relies on them: the decode
+//    always runs PHASE_PRE, whose first kernel (k_index) resets the status words, cursors and the queue count, and the
+//    chain / barrier counters are cleared by the launches that use them — exactly as with a caller's uninitialised scratch.
+//  * Calls that overlap on the GPU (two streams, two plans, two host threads) race on the array: one call at a time per
+//    device; aceapex_get_stats_noalloc must be called before the next aceapex_decode_noalloc on that device.
+namespace {
+constexpr size_t NOALLOC_MAX = (size_t)16 << 20;     // 16 MiB: a stream of up to ~1.4 M sequences (config 0, 4 MB, needs 5.6 MB)
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static __device__ __align__(256) unsigned char ax_noalloc_scratch[NOALLOC_MAX];
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[NOALLOC_MAX_DEVICES];            // device address of ax_noalloc_scratch, per device ordinal (0 = not set up)
+
+// Set-up, once per device, with that device current.
+cudaError_t noalloc_scratch(int device, void** out) {
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[device]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, ax_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr || ((uintptr_t)ptr & 255)) return cudaErrorInvalidSymbol;
+        g_noalloc_ptr[device] = ptr;
+    }
+    *out = g_noalloc_ptr[device];
+    return cudaSuccess;
+}
+}  // namespace
+
+extern "C" size_t aceapex_noalloc_max_scratch_bytes(void) { return NOALLOC_MAX; }
+
+extern "C" int aceapex_decode_noalloc(aceapex_plan_t* p, const void* comp_dev, void* out_dev, size_t out_capacity, void* stream) {
+    if (!p) return ACEAPEX_E_ARG;
+    if (p->scratch_bytes > NOALLOC_MAX) return ACEAPEX_E_NOALLOC_LIMIT;          // stated maximum: rejected, nothing launched
+    if (p->n_blocks == 0) { p->last_launches = 0; p->last_stream = (cudaStream_t)stream; return ACEAPEX_OK; }
+    if (!comp_dev || !out_dev) return ACEAPEX_E_ARG;
+    if (out_capacity < aceapex_out_bytes(p)) return ACEAPEX_E_CAPACITY;
+    if (((uintptr_t)comp_dev | (uintptr_t)out_dev) & 15) return ACEAPEX_E_ALIGN;
+    int cur = -1;
+    cudaError_t e = cudaGetDevice(&cur);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+    if (cur != p->device) return ACEAPEX_E_ARG;                                   // kernel attributes / grids belong to the plan's device
+    void* scratch = nullptr;
+    e = noalloc_scratch(cur, &scratch);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; cudaGetLastError(); return ACEAPEX_E_CUDA; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int strategy = p->strategy_forced != ACEAPEX_WAVES_AUTO ? p->strategy_forced : p->strategy_auto;
+    if (strategy == ACEAPEX_WAVES_GRAPH) strategy = ACEAPEX_WAVES_LAUNCH;        // (instantiating a graph allocates)
+    p->last_stream = st; p->last_strategy = strategy; p->last_had_match = true;
+    const Params P = make_params(p, comp_dev, out_dev, scratch, strategy);
+    e = enqueue(p, P, ACEAPEX_PHASE_ALL, strategy, st, &p->last_launches);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; return ACEAPEX_E_CUDA; }
+    return ACEAPEX_OK;
+}
+
+extern "C" int aceapex_get_stats_noalloc(aceapex_plan_t* p, aceapex_stats* s) {
+    if (!p || !s) return ACEAPEX_E_ARG;
+    void* scratch = nullptr;
+    if (p->n_blocks) {
+        int cur = -1;
+        cudaError_t e = cudaGetDevice(&cur);
+        if (e == cudaSuccess && cur != p->device) return ACEAPEX_E_ARG;
+        if (e == cudaSuccess) e = noalloc_scratch(cur, &scratch);
+        if (e != cudaSuccess) { p->last_cuda = (int)e; cudaGetLastError(); return ACEAPEX_E_CUDA; }
+    }
+    return aceapex_get_stats(p, scratch, s);
 }
