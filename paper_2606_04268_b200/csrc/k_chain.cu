@@ -9,10 +9,11 @@
 //   a2  the tile's cmd[] / len[] / dep[] / off[] slices and its slice of lit[] arrive in shared memory by 1-D bulk TMA
 //       (cp.async.bulk + mbarrier), two stages: the tile after next is in flight; its descriptor is fetched by one thread
 //       (cp.async) meanwhile
-//   a3  scan inside the tile: each thread sums 2 CONSECUTIVE sequences, warp shuffles + one barrier give every token's
-//       output position and literal offset (the tile's prefix inside its block comes from k_tilesum), kept in shared memory
-//   a6  then thread t takes tokens t, t+256 (neighbouring lanes = neighbouring tokens: neighbouring sources share L1
-//       lines, neighbouring destinations share image words):
+//   a3  scan inside the tile: thread t owns sequences 2t and 2t+1 through every phase (what it learns about them stays in
+//       registers); warp shuffles + one barrier give every token's output position and literal offset (the tile's prefix
+//       inside its block comes from k_tilesum)
+//   a6  neighbouring lanes hold neighbouring tokens (neighbouring sources share L1 lines, neighbouring destinations share
+//       image words):
 //         before the wait  literal runs go into a shared-memory IMAGE of the tile's output span; each match is reduced to
 //                          (aligned source address, destination, length / phase / period)
 //         gather           the aligned 8-byte words holding each match's source travel global -> shared with cp.async
@@ -21,8 +22,9 @@
 //                          one owner: no merge, no zero fill), periodic if it overlaps its source (Q3); matches
 //                          up to 32 bytes by one thread, longer ones by the whole warp
 //       and the image goes to global memory with coalesced 16-byte vector stores (<= 15 head / tail bytes by byte stores;
-//       measured against one bulk TMA store + its completion wait: 7.2 vs 7.7 ms on fastq1g — the wait is on the chain).  Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight
-//       to global memory instead (their literal runs are there already: the literal scatter ran before).
+//       measured against one bulk TMA store + its completion wait: 7.2 vs 7.7 ms on fastq1g — the wait is on the chain).
+//       Tokens that would end beyond the image capacity (tiles with long matches / runs) are written straight to global
+//       memory instead (their literal runs are there already: the literal scatter ran before).
 // Rewriting a literal byte with its own value while another CTA reads it as a match source is harmless: a reader sees the
 // old or the new copy of the same value.
 #include "common.cuh"
@@ -35,8 +37,9 @@ constexpr int SP_PER = 2;                            // tokens per thread (measu
                                                      // and a 512-sequence tile spreads a block's ~370 tiles over all SMs: 7.1 us)
 constexpr int SP_THREADS = TILE / SP_PER;            // 256
 constexpr int SP_WARPS = SP_THREADS / 32;
-constexpr int SP_OCC = 3;                            // CTAs per SM (85 registers per thread: measured 7.7 / 8.05 / 10.3 ms on fastq1g
-                                                     // for 3 / 4 / 5 CTAs — the register cap costs more than residency gains)
+constexpr int SP_OCC = 3;                            // CTAs per SM (77 registers per thread: measured 9.80 / 6.40 / 6.84 ms on fastq1g
+                                                     // for 2 / 3 / 4 CTAs — at 4 the 64-register cap spills; at 2 less than one
+                                                     // block's tiles are resident)
 constexpr uint32_t SP_STRM = TILE * 10u;             // cmd | len | dep (2 B each) | off (4 B) per sequence
 constexpr uint32_t SP_O_LEN = TILE * 2u, SP_O_DEP = TILE * 4u, SP_O_OFF = TILE * 6u;
 constexpr uint32_t SP_IMG = 10 * TILE;               // image capacity in bytes (a text / FASTQ tile of 512 sequences spans ~3 KB)
