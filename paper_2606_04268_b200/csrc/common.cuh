@@ -65,7 +65,7 @@ struct Params {
     BlockDesc* blocks;                             // [n_blocks]
     unsigned long long* tile_state;                // [n_tiles] exclusive (out << 32 | lit) prefix of the tile inside its block
     uint32_t* tile_blk;                            // [n_tiles] block index of the tile
-    uint32_t* chain_sync;                          // strategy CHAIN: [0] frontier, [32 + b] finished tiles of block b
+    uint32_t* chain_sync;                          // strategy CHAIN: [32 + b] finished tiles of block b (complete only once blocks < b are)
     uint4* lit_q;                                  // [lit_q_cap] long literal runs: (dst, len, src offset in comp lo, hi)
     uint32_t lit_q_cap;
     uint32_t long_runs;                            // the header's mean literal run is 4-20 bytes (picks the literal pass instance)

@@ -3,7 +3,7 @@
 // After chain flattening no match reads bytes produced by another match of its own block (§3.3, invariant
 // I3), so once the literal scatter has run, every match of block b depends on blocks < b only.  Tiles are taken in file
 // order; a tile that holds a match of depth > 1 with a source before its block waits until every earlier block is
-// completely written (a7: per-block completion counts + a frontier word instead of one grid barrier per depth —
+// completely written (a7: per-block completion counts instead of one grid barrier per depth —
 // PAPER.md:224 "synchronization-bound"); dep[] is used only to skip the wait (dep == 1: all sources are literals).
 // Per tile (512 sequences of one block, 256 threads, 3 CTAs per SM):
 //   a2  the tile's cmd[] / len[] / dep[] / off[] slices and its slice of lit[] arrive in shared memory by 1-D bulk TMA
@@ -53,7 +53,7 @@ static_assert(SP_THREADS % 32 == 0 && SP_THREADS <= 1024 && SP_THREADS * SP_PER 
 struct TileMeta {
     unsigned long long pre;                          // (out << 32 | lit) prefix of the tile inside its block
     const uint8_t* lit;                              // the block's lit[] in global memory
-    uint32_t b, blk_lo, nt, blk_tiles, prev_tiles;   // block, its first output byte, sequences in the tile, tiles of blocks b and b-1
+    uint32_t b, blk_lo, nt, prev_tiles;              // block, its first output byte, sequences in the tile, tiles of block b-1
     uint32_t lit16, lit_ok;                          // slit[0] = lit[lit16]; lit_ok: the tile's literal bytes are staged
 };
 
@@ -137,7 +137,7 @@ __device__ __forceinline__ void issue_tile_loads(const Params& P, SpanSmem& S, u
     const bool lit_ok = lbytes <= SP_LIT;
     TileMeta& M = S.meta[st];
     M.pre = F.pre; M.lit = P.comp + F.B.lit_off; M.b = F.b; M.blk_lo = (uint32_t)F.B.out_base; M.nt = n;
-    M.blk_tiles = (F.B.n_seq + TILE - 1) / TILE; M.prev_tiles = (F.prev_tiles + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
+    M.prev_tiles = (F.prev_tiles + TILE - 1) / TILE; M.lit16 = l16; M.lit_ok = lit_ok ? 1u : 0u;
     const uint32_t b2 = (uint32_t)pad16(2ull * n), b4 = (uint32_t)pad16(4ull * n);
     mbar_expect_tx(&S.mbar[st], 3 * b2 + b4 + (lit_ok ? lbytes : 0u));
     bulk_load(S.strm[st], P.comp + F.B.cmd_off + 2ull * j0, b2, &S.mbar[st]);
@@ -154,8 +154,8 @@ __device__ __forceinline__ V16 extract16(unsigned long long x0, unsigned long lo
     return v;
 }
 
-// chain_sync[0] = frontier word (blocks 0 .. frontier-1 are completely written; trails the truth by up to one hop);
-// chain_sync[32 + b] = finished tiles of block b (block b is complete when it reaches the block's tile count)
+// chain_sync[32 + b] = finished tiles of block b.  It reaches the block's tile count only when blocks 0 .. b are ALL complete
+// (words 0 .. 31 are unused padding: the counts start on their own 128-byte line)
 constexpr uint32_t CH_CNT0 = 32;
 
 __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
@@ -191,7 +191,7 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
         const TileMeta& M = S.meta[st];
         const unsigned long long pre = M.pre;
         const uint8_t* const lit = M.lit;
-        const uint32_t b = M.b, blk_lo = M.blk_lo, nt = M.nt, blk_tiles = M.blk_tiles, prev_tiles = M.prev_tiles;
+        const uint32_t b = M.b, blk_lo = M.blk_lo, nt = M.nt, prev_tiles = M.prev_tiles;
         const uint8_t* const lsrc_base = M.lit_ok ? S.slit[st] - M.lit16 : lit;   // byte x of the block's lit[] is lsrc_base[x]
         uint16_t* const s_cmd = reinterpret_cast<uint16_t*>(S.strm[st]);
         uint16_t* const s_len = reinterpret_cast<uint16_t*>(S.strm[st] + SP_O_LEN);
@@ -284,24 +284,20 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
             }
         }
         if (tid == 0 && has_next) fetch_step2(P, F);                       // (its block index has arrived by now)
-        if (must_wait) {
-            // a7: every block before this one completely written?  One thread spins; its acquire also drops this SM's L1
-            // (CCTL.IVALL), so the loads below see what other SMs wrote.
+        if (must_wait && b) {
+            // a7: every block before this one completely written?  count[b-1] reaches the tile count of block b-1 only when
+            // blocks 0 .. b-1 are all complete (a tile publishes only after it has seen block b-2's count complete: here, or
+            // before its publish below), so this one word is the whole condition.  One thread spins; the poll itself is the
+            // acquire (SASS: LDG.STRONG.GPU + CCTL.IVALL, which also drops this SM's L1 so that the gathers below see what
+            // other SMs wrote): a relaxed poll followed by fence.acq_rel.gpu puts a MEMBAR.ALL.GPU in front of the gathers
+            // (measured 6.70 vs 6.39 ms per decode on fastq1g).
             if (tid == 0) {
-                // blocks 0 .. b-2: the frontier word (moved by the last tile of every block, in block order, one hop ago);
-                // block b-1: its completion count itself, so that the returning atomic and the frontier store of its last
-                // tile are off the critical path
                 uint32_t v;
                 for (;;) {
-                    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory");
-                    if (v + 1u >= b) break;
-                    __nanosleep(400);                                     // not next in line: keep the hot lines' queues short
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory");
+                    if (v >= prev_tiles) break;
+                    if (v == 0) __nanosleep(400);                         // block b-1 has not begun to finish: keep the hot line's queue short
                 }
-                // the poll itself is the acquire (SASS: LDG.STRONG.GPU + CCTL.IVALL): a relaxed poll followed by fence.acq_rel.gpu
-                // puts a MEMBAR.ALL.GPU in front of the gathers — measured 6.70 vs 6.39 ms per decode on fastq1g
-                if (v < b) {
-                    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory"); } while (v < prev_tiles);
-                } else asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory");
             }
             __syncthreads();                                              // barrier 2
         }
@@ -375,13 +371,13 @@ __global__ void __launch_bounds__(SP_THREADS, SP_OCC) k_chain(Params P) {
             }
             __syncthreads();                                              // barrier 5: every store of the tile is issued
             if (tid == 0) {
-                uint32_t old;
-                asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
-                if (old + 1u == blk_tiles) {
+                // publish.  A tile that did not have to wait still may not count before blocks < b are complete (see the
+                // wait above: count[b] complete must imply that); it has normally long been the case.
+                if (!must_wait && b) {
                     uint32_t v;
-                    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync) : "memory"); } while (v < b);
-                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(P.chain_sync), "r"(b + 1u) : "memory");
+                    do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(P.chain_sync + CH_CNT0 + b - 1u) : "memory"); } while (v < prev_tiles);
                 }
+                asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(P.chain_sync + CH_CNT0 + b), "r"(1u) : "memory");
             }
         }
     }
@@ -406,7 +402,7 @@ int chain_max_ctas_per_sm() {
 }
 
 // Every tile of the grid must be resident (a tile spins until lower tiles are done), so the launch is cooperative and the
-// grid at most n_sm x occupancy; the frontier word and the per-block counts start from zero.
+// grid at most n_sm x occupancy; the per-block counts start from zero.
 cudaError_t launch_chain(const Params& P, int grid, cudaStream_t st) {
     if (!P.n_tiles) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(P.chain_sync, 0, sizeof(uint32_t) * (CH_CNT0 + (size_t)P.n_blocks), st);
