@@ -85,9 +85,9 @@ extern "C" const char* aceapex_strerror(int code) {
 //   PASSES      literal pass 6.1 ps/seq (7.5 when it lists sparse depths) + per dense depth one streaming pass 3.6 ps/seq
 //               (+ ~3 us launch) + 8.8 ps per match copied; per sparse depth one list wave (5.5 us + 21 ps per match)
 //   LAUNCH      bucketing pass (k_pre) 14.5 ps/seq + per non-empty depth one launch ~5.5 us + 21 ps per match copied from a list
-//   PERSISTENT  the same lists, one cooperative kernel: ~4 us of grid barrier + fence drain + straggler wait per depth
+//   PERSISTENT  the same lists, one cooperative kernel: ~3.6 us of grid barrier + fence drain + straggler wait per depth
 //   CHAIN       (FLATTENED streams only) literal pass 3.1 ps/seq, then one pass whose time is the larger of the block chain
-//               (one ~6.5 us hop per 1 MB block) and its issue-bound throughput (26 ps/seq)
+//               (one ~5.5 us hop per 1 MB block) and its issue-bound throughput (26 ps/seq)
 // PASSES is limited to PASS_MAX_DEPTH waves.
 static int choose_strategy(const aceapex_plan_t* p) {
     if (p->max_depth == 0) return ACEAPEX_WAVES_LAUNCH;
@@ -95,14 +95,14 @@ static int choose_strategy(const aceapex_plan_t* p) {
     for (uint32_t d = 1; d <= p->max_depth; ++d) waves += p->hist_cnt[d] != 0;
     const double seq = (double)p->total_seq, m = (double)p->n_match;
     const double t_lists = 14.5e-6 * seq + 21e-6 * m;                           // microseconds
-    const double t_launch = t_lists + 5.5 * waves, t_persist = t_lists + 4.0 * waves + 8.0;
+    const double t_launch = t_lists + 5.5 * waves, t_persist = t_lists + 3.6 * waves + 8.0;
     double t_passes = 1e300;
     if (p->max_depth <= PASS_MAX_DEPTH) {
         t_passes = (p->list_mask ? 7.5e-6 : 6.1e-6) * seq;                     // literal pass (+ listing the sparse depths)
         for (uint32_t d = 1; d <= p->max_depth; ++d)
             t_passes += ((p->list_mask >> d) & 1u) ? 5.5 + 21e-6 * (double)p->hist_cnt[d] : 3.0 + 3.6e-6 * seq + 8.8e-6 * (double)p->hist_cnt[d];
     }
-    const double hop = 6.5 * p->n_blocks, thr = 26e-6 * seq;
+    const double hop = 5.5 * p->n_blocks, thr = 26e-6 * seq;
     const double t_chain = (p->flags & FLAG_FLATTENED) ? 3.1e-6 * seq + (hop > thr ? hop : thr) + 10.0 : 1e300;
     int best = ACEAPEX_WAVES_LAUNCH; double t = t_launch;
     if (t_persist < t) { best = ACEAPEX_WAVES_PERSISTENT; t = t_persist; }
