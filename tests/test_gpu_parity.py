@@ -138,7 +138,9 @@ CASES = [("markov", 1 << 20, dict(block_size=1 << 18)),
          ("stress", 4 << 20, dict(depth_limit=1)),
          ("text", 3 << 20, dict(min_match=11)),                                          # token-cost-aware regime (Q4):
          ("fastq", (3 << 20) + 5, dict(min_match=11, depth_limit=4)),                    # long literal runs, fewer and longer matches
-         ("fastq", 2 << 20, dict(min_match=11, max_chain=4, flatten=False))]
+         ("fastq", 2 << 20, dict(min_match=11, max_chain=4, flatten=False)),
+         ("text", 16 << 20, dict(block_size=8 << 20, max_chain=4)),      # ~1900 tiles per block: more than k_chain keeps resident
+         ("markov", 1 << 20, dict(block_size=4096))]                     # 256 blocks of one tile each: one chain hop per tile
 
 
 @pytest.mark.parametrize("kind,n,kw", CASES)
