@@ -27,6 +27,8 @@ struct PassSmem {
     unsigned long long warp_sum[PS_WARPS];
     uint32_t cnt;                                        // matches this CTA copied in this pass (histogram check)
     uint32_t lcnt[PASS_MAX_DEPTH + 1], lbase[PASS_MAX_DEPTH + 1];   // literal pass: the tile's listed matches per sparse depth, their list slots
+    uint32_t lloc[PASS_MAX_DEPTH + 1], nloc;             // ... and their places in the tile's staging area (w_dst / w_off / w_len / e_g)
+    uint32_t e_g[TILE_STREAM];                           // list slot of every staged entry
     uint32_t w_dst[PS_WARPS][PS_WCAP];                   // per warp: the tile's matches of this pass, compacted
     uint32_t w_off[PS_WARPS][PS_WCAP];
     uint16_t w_len[PS_WARPS][PS_WCAP];
@@ -44,6 +46,7 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
     if (tid == 0) S.cnt = 0;
     constexpr bool listing = LIT && LISTING;                        // some depths are sparse: their matches are listed here
     if (listing && tid <= PASS_MAX_DEPTH) S.lcnt[tid] = 0;
+    if (listing && tid == 0) S.nloc = 0;
     __syncthreads();
     for (uint32_t tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
         const uint32_t b = P.tile_blk[tile];
@@ -127,23 +130,37 @@ __global__ void __launch_bounds__(PS_THREADS, 1024 / PS_THREADS) k_pass(Params P
                 pos += c[k] + l[k]; lsrc += c[k];
             }
             if (listing) {
-                // a5 for the sparse depths only: reserve the tile's slice of each depth's wave list, write the entries
+                // a5 for the sparse depths only: reserve the tile's slice of each depth's wave list, group the tile's entries by
+                // depth in shared memory (the staging arrays of the match passes are idle here), then write them out in list
+                // order so that consecutive threads store consecutive slots (as k_pre does: coalesced runs, one per depth)
+                uint32_t* const e_dst = &S.w_dst[0][0]; uint32_t* const e_off = &S.w_off[0][0]; uint16_t* const e_len = &S.w_len[0][0];
                 __syncthreads();
-                if (tid <= PASS_MAX_DEPTH && S.lcnt[tid]) S.lbase[tid] = atomicAdd(&P.cursor[tid], S.lcnt[tid]);
+                if (tid <= PASS_MAX_DEPTH && S.lcnt[tid]) {
+                    S.lbase[tid] = atomicAdd(&P.cursor[tid], S.lcnt[tid]);
+                    S.lloc[tid] = atomicAdd(&S.nloc, S.lcnt[tid]);
+                }
                 __syncthreads();
                 uint32_t p2 = pos0;
 #pragma unroll
                 for (int k = 0; k < PRE_ITEMS; ++k) {
                     p2 += c[k];
                     if (sel_mask & (1u << k)) {
-                        const uint32_t g = S.lbase[dp[k]] + rank[k];
-                        if (g < P.wave_off[dp[k] + 1]) { P.wl_dst[g] = blk_lo + p2; P.wl_off[g] = of[k]; P.wl_len[g] = (uint16_t)l[k]; }
-                        else raise_fault(P.status, F_DEPTH, b);      // more matches than the histogram says
+                        const uint32_t i = S.lloc[dp[k]] + rank[k];
+                        uint32_t g = S.lbase[dp[k]] + rank[k];
+                        if (g >= P.wave_off[dp[k] + 1]) { raise_fault(P.status, F_DEPTH, b); g = 0xFFFFFFFFu; }   // more matches than the histogram says
+                        e_dst[i] = blk_lo + p2; e_off[i] = of[k]; e_len[i] = (uint16_t)l[k]; S.e_g[i] = g;
                     }
                     p2 += l[k];
                 }
                 __syncthreads();
+                const uint32_t nloc = S.nloc;
+                for (uint32_t i = tid; i < nloc; i += PS_THREADS) {
+                    const uint32_t g = S.e_g[i];
+                    if (g != 0xFFFFFFFFu) { P.wl_dst[g] = e_dst[i]; P.wl_off[g] = e_off[i]; P.wl_len[g] = e_len[i]; }
+                }
+                __syncthreads();
                 if (tid <= PASS_MAX_DEPTH) S.lcnt[tid] = 0;          // (ordered before the next tile's counting by its scan barriers)
+                if (tid == 0) S.nloc = 0;
             }
         } else {
             // ---- a6: select this pass's matches (same validity rule as pass 0), compact them per warp, copy
